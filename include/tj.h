@@ -1,0 +1,136 @@
+/*
+ * tj.h -- C ABI of libtj: pseudo-C_ell mode-coupling matrices on one B200 (sm_100a), FP64.
+ *
+ * Method: arxiv/paper_2602_15605, "threej_cosmo": Wigner-3j symbols from a few
+ * recurrence-generated lookup tables (PAPER.md:161-186 Eqs. 10-12; :188-220 Eqs. 13-16; App. B)
+ * instead of a per-pair Schulten-Gordon recursion.  The formula sheet the kernels implement is
+ * DESIGN.md section 3 (= SURVEY.md 8(c.1)).
+ *
+ * Conventions (all entry points)
+ *   - Pointers named d_* are DEVICE pointers owned by the caller; h_* are HOST pointers.  The library
+ *     never frees caller memory and never keeps a caller pointer after the call's work has been
+ *     enqueued.  Outputs are fully overwritten (no accumulate mode).
+ *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  All work is
+ *     enqueued on it and the call returns without synchronising, except where stated.
+ *   - Matrices are row-major float64, row index l1, column index l2, including l = 0 and 1:
+ *     M[l1*(lmax+1) + l2] = K_{l1 l2} = (2 l2+1) Xi(l1,l2)          (PAPER.md:76 Eq. 3, :328).
+ *     Rows/columns l < 2 of the polarised blocks (TE, EE, BB, EB) are exactly 0.0.
+ *   - Windows are float64 W_l, l = 0..nW-1.  The l3 sum runs over |l1-l2| <= l3 <= min(l1+l2, l3max)
+ *     (PAPER.md:226: W_L is needed for L <= 2 lmax; :251: stopping earlier is exact when W vanishes beyond).
+ *   - Every call returns TJ_OK (0) or a negative code; no exceptions, no aborts, no errno.
+ *   - There is no CPU fallback: without a CUDA device every compute entry point returns TJ_ECUDA.
+ */
+#ifndef TJ_H_
+#define TJ_H_
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define TJ_OK       0
+#define TJ_EINVAL  (-1)  /* bad argument: negative sizes, l3max > 2*lmax, nW mismatch, NULL required pointer,
+                            an output requested without its window */
+#define TJ_ENOMEM  (-2)  /* host or device allocation failed */
+#define TJ_ECUDA   (-3)  /* CUDA runtime / launch error; text via tj_strerror(TJ_ECUDA) */
+
+/* Opaque handle owning the device-resident lookup tables for one (lmax, l3max).  Immutable after
+ * build, so it may be used concurrently from several streams. */
+typedef struct tj_tables tj_tables;
+
+/*
+ * tj_build_tables -- lookup-table build kernel (Eqs. 11-12).
+ *   g(p) = (p - 1/2)/p * g(p-1), g(0) = 1, for p = 0..2*lmax+1, carried in double-double so every
+ *   stored double is the faithfully rounded value of Eq. 11; plus the folded tables of DESIGN.md 3:
+ *   ginv = 1/g, h = 1/((2p+1) g)  [the 1/(J+1) table of PAPER.md:186 at J = 2p, folded into 1/g],
+ *   gA = 2p g, gB = (2p+1) g [odd-J branch], all with zero guard bands, and the per-l constants
+ *   u_l = l(l+1), 1/sqrt((l-1)l(l+1)(l+2)).
+ *   lmax  >= 0; 0 <= l3max <= 2*lmax.  Enqueues on `cuda_stream` and synchronises it once.
+ *   *out receives the handle (free with tj_free_tables).
+ */
+int tj_build_tables(int lmax, int l3max, void *cuda_stream, tj_tables **out);
+void tj_free_tables(tj_tables *tables);
+
+/* Sizes held by a handle.  Any output pointer may be NULL. */
+int tj_tables_info(const tj_tables *tables, int *lmax, int *l3max, int *pmax);
+
+/*
+ * tj_tables_copy -- copy one table to HOST memory (synchronous; for tests of the table kernel).
+ *   which: 0 g, 1 ginv, 2 h, 3 gA, 4 gB  (count <= pmax+1 entries, p = 0..count-1);
+ *          5 u_l, 6 1/sqrt(D_l)          (count <= lmax+1 entries).
+ */
+int tj_tables_copy(const tj_tables *tables, int which, double *h_dst, int count);
+
+/*
+ * tj_coupling_tt -- K^{TT} (PAPER.md:76-78 Eq. 3; :340 Eq. A1) with the squared (000) symbol from
+ * Eq. 10.  d_Wtt: nW = l3max+1 entries.  d_TT: (lmax+1)^2 doubles.
+ */
+int tj_coupling_tt(const tj_tables *tables, const double *d_Wtt, int nW, double *d_TT, void *cuda_stream);
+
+/*
+ * tj_coupling_pol -- all blocks in ONE fused l3 sweep (PAPER.md:80-84 Eq. 4; :340-356 Eqs. A1-A4;
+ * spin-2 symbol from Eqs. 13-16 / B14-B17 in the one-product form of DESIGN.md 3).
+ *   TT needs d_Wtt; TE needs d_Wtp; EE, BB, EB need d_Wpp.  Any output may be NULL (skipped); a window
+ *   may be NULL iff none of its outputs is requested.  BB is a copy of EE.
+ *   Each window: nW = l3max+1 entries.  Each output: (lmax+1)^2 doubles.
+ */
+int tj_coupling_pol(const tj_tables *tables,
+                    const double *d_Wtt, const double *d_Wtp, const double *d_Wpp, int nW,
+                    double *d_TT, double *d_TE, double *d_EE, double *d_BB, double *d_EB,
+                    void *cuda_stream);
+
+/*
+ * tj_coupling_band -- band-limited variant: the l3 sum stops at lcut (inclusive),
+ * exact when W_l = 0 for l > lcut.  0 <= lcut <= 2*lmax of the handle.
+ *   Windows: lcut+1 entries each.  Outputs: banded storage, (lmax+1)*(2*lcut+1) doubles each,
+ *   band[l1*(2*lcut+1) + (l2-l1+lcut)] = K_{l1 l2} for |l1-l2| <= lcut and 0 <= l2 <= lmax; slots whose
+ *   l2 falls outside 0..lmax are written 0.0.  NULL rules as tj_coupling_pol.
+ */
+int tj_coupling_band(const tj_tables *tables, int lcut,
+                     const double *d_Wtt, const double *d_Wtp, const double *d_Wpp,
+                     double *d_TT, double *d_TE, double *d_EE, double *d_BB, double *d_EB,
+                     void *cuda_stream);
+
+/*
+ * Host-buffer forms (the end-to-end path): same semantics, but every window and output is a HOST
+ * pointer (h_*; pinned memory makes the copies asynchronous and fast, pageable memory also works).
+ * The call allocates device scratch from the stream-ordered pool, copies the windows in, runs the same
+ * kernels, copies every requested matrix back and SYNCHRONISES the stream before returning.
+ * band = 0: dense outputs, nW_or_lcut = nW = l3max+1;  band = 1: banded outputs, nW_or_lcut = lcut.
+ */
+int tj_coupling_host(const tj_tables *tables, int band, int nW_or_lcut,
+                     const double *h_Wtt, const double *h_Wtp, const double *h_Wpp,
+                     double *h_TT, double *h_TE, double *h_EE, double *h_BB, double *h_EB,
+                     void *cuda_stream);
+
+/*
+ * tj_l3_range -- host-side integer bookkeeping of the l3 sum for one pair: l3 runs over
+ * |l1-l2|..min(l1+l2, l3max) with (l1+l2+l3)%2 == parity (0: TT/TE/EE/BB, 1: EB).
+ * nterms may be 0 (then *l3_lo > *l3_hi).  Output pointers may be NULL.
+ */
+int tj_l3_range(int l1, int l2, int l3max, int parity, int *l3_lo, int *l3_hi, int *nterms);
+
+/*
+ * tj_sweep_counts -- the number of l3 terms the sweep kernel evaluates for one pair as the KERNEL
+ * walks them (first/last step index t of the even and odd branch), so tests can check the
+ * kernel's loop bounds against tj_l3_range / the oracle bit-exactly.  Host-side.
+ *   even: l3 = l1+l2-2t, t = *te_lo..*te_hi;   odd: l3 = l1+l2-2t-1, t = *to_lo..*to_hi.
+ */
+int tj_sweep_counts(int l1, int l2, int l3max, int *te_lo, int *te_hi, int *to_lo, int *to_hi);
+
+/*
+ * tj_fp64_probe -- measurement aid for the roofline denominator: runs `iters` dependent-chain DFMA
+ * iterations of 8 independent chains per thread on every SM and returns, through *h_thread_instr_per_s,
+ * the achieved FP64 thread-instructions per second (synchronous; CUDA-event timed).
+ */
+int tj_fp64_probe(int iters, void *cuda_stream, double *h_thread_instr_per_s);
+
+/* Time of the last-enqueued work is the caller's to measure; this returns how many kernels the given
+ * entry point launches per call (for bench.py's gpu_launches): which = 0 tt, 1 pol, 2 band. */
+int tj_launches_per_call(int which);
+
+const char *tj_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TJ_H_ */

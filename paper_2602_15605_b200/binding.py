@@ -1,0 +1,234 @@
+"""Thin Python binding of libtj (include/tj.h): argument marshalling only.
+
+Every step of the path runs in the library's CUDA kernels; this file converts torch tensors to
+device pointers, picks the current CUDA stream and turns error codes into exceptions.  There is
+no fallback of any kind: if `libtj.so` is missing or a call fails, a TJError is raised.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SO = os.path.join(_HERE, "libtj.so")
+_LIB = None
+
+TJ_OK, TJ_EINVAL, TJ_ENOMEM, TJ_ECUDA = 0, -1, -2, -3
+
+# every symbol include/tj.h declares (tests/test_abi.py checks the header against this and the .so)
+SYMBOLS = (
+    "tj_build_tables", "tj_free_tables", "tj_tables_info", "tj_tables_copy",
+    "tj_coupling_tt", "tj_coupling_pol", "tj_coupling_band", "tj_coupling_host",
+    "tj_l3_range", "tj_sweep_counts", "tj_fp64_probe", "tj_launches_per_call", "tj_strerror",
+)
+
+
+class TJError(RuntimeError):
+    def __init__(self, code, what):
+        self.code = code
+        super().__init__("%s failed: %s (code %d)" % (what, _strerror(code), code))
+
+
+def library_path() -> str:
+    return _SO
+
+
+def load_library() -> ctypes.CDLL:
+    """Load libtj.so (built in-tree by `python -m paper_2602_15605_b200.build`).  Fails loudly."""
+    global _LIB
+    if _LIB is not None:
+        return _LIB
+    if not os.path.exists(_SO):
+        raise TJError(TJ_ECUDA, "loading %s (not built: run `python -m paper_2602_15605_b200.build`; "
+                                "there is no CPU fallback)" % _SO)
+    L = ctypes.CDLL(_SO)
+    vp, ip, dp, ci = ctypes.c_void_p, ctypes.POINTER(ctypes.c_int), ctypes.POINTER(ctypes.c_double), ctypes.c_int
+    L.tj_build_tables.argtypes = [ci, ci, vp, ctypes.POINTER(vp)]
+    L.tj_free_tables.argtypes = [vp]
+    L.tj_free_tables.restype = None
+    L.tj_tables_info.argtypes = [vp, ip, ip, ip]
+    L.tj_tables_copy.argtypes = [vp, ci, dp, ci]
+    L.tj_coupling_tt.argtypes = [vp, vp, ci, vp, vp]
+    L.tj_coupling_pol.argtypes = [vp, vp, vp, vp, ci, vp, vp, vp, vp, vp, vp]
+    L.tj_coupling_band.argtypes = [vp, ci, vp, vp, vp, vp, vp, vp, vp, vp, vp]
+    L.tj_coupling_host.argtypes = [vp, ci, ci, vp, vp, vp, vp, vp, vp, vp, vp, vp]
+    L.tj_l3_range.argtypes = [ci, ci, ci, ci, ip, ip, ip]
+    L.tj_sweep_counts.argtypes = [ci, ci, ci, ip, ip, ip, ip]
+    L.tj_fp64_probe.argtypes = [ci, vp, dp]
+    L.tj_launches_per_call.argtypes = [ci]
+    L.tj_strerror.argtypes = [ci]
+    L.tj_strerror.restype = ctypes.c_char_p
+    for name in SYMBOLS:
+        if name not in ("tj_free_tables", "tj_strerror"):
+            getattr(L, name).restype = ci
+    _LIB = L
+    return L
+
+
+def _strerror(code):
+    try:
+        return load_library().tj_strerror(code).decode()
+    except Exception:
+        return {TJ_EINVAL: "invalid argument", TJ_ENOMEM: "out of memory", TJ_ECUDA: "CUDA error"}.get(code, "?")
+
+
+def _check(code, what):
+    if code != TJ_OK:
+        raise TJError(code, what)
+
+
+def _stream_ptr(stream=None):
+    import torch
+    s = torch.cuda.current_stream() if stream is None else stream
+    return ctypes.c_void_p(s.cuda_stream)
+
+
+def _dev_ptr(t, n, name):
+    """Device pointer of a contiguous float64 CUDA tensor with n elements (None -> NULL)."""
+    import torch
+    if t is None:
+        return ctypes.c_void_p(0)
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()):
+        raise TJError(TJ_EINVAL, "%s must be a contiguous float64 CUDA tensor" % name)
+    if t.numel() != n:
+        raise TJError(TJ_EINVAL, "%s must have %d elements, has %d" % (name, n, t.numel()))
+    return ctypes.c_void_p(t.data_ptr())
+
+
+def _host_ptr(t, n, name):
+    import torch
+    if t is None:
+        return ctypes.c_void_p(0)
+    if not (isinstance(t, torch.Tensor) and (not t.is_cuda) and t.dtype == torch.float64 and t.is_contiguous()):
+        raise TJError(TJ_EINVAL, "%s must be a contiguous float64 CPU tensor" % name)
+    if t.numel() != n:
+        raise TJError(TJ_EINVAL, "%s must have %d elements, has %d" % (name, n, t.numel()))
+    return ctypes.c_void_p(t.data_ptr())
+
+
+class Tables:
+    """Owns a tj_tables handle (tj_build_tables / tj_free_tables)."""
+
+    def __init__(self, lmax: int, l3max: int | None = None, stream=None):
+        L = load_library()
+        self.lmax = int(lmax)
+        self.l3max = 2 * self.lmax if l3max is None else int(l3max)
+        h = ctypes.c_void_p()
+        _check(L.tj_build_tables(self.lmax, self.l3max, _stream_ptr(stream), ctypes.byref(h)), "tj_build_tables")
+        self._h = h
+        a, b, c = ctypes.c_int(), ctypes.c_int(), ctypes.c_int()
+        _check(L.tj_tables_info(self._h, ctypes.byref(a), ctypes.byref(b), ctypes.byref(c)), "tj_tables_info")
+        self.pmax = c.value
+
+    @property
+    def handle(self):
+        return self._h
+
+    def copy_table(self, which: int, count: int):
+        import numpy as np
+        out = np.empty(count, dtype=np.float64)
+        _check(load_library().tj_tables_copy(self._h, which, out.ctypes.data_as(ctypes.POINTER(ctypes.c_double)), count),
+               "tj_tables_copy")
+        return out
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            load_library().tj_free_tables(self._h)
+            self._h = ctypes.c_void_p(0)
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def build_tables(lmax: int, l3max: int | None = None, stream=None) -> Tables:
+    return Tables(lmax, l3max, stream)
+
+
+def coupling_tt(tables: Tables, Wtt, TT=None, stream=None):
+    """tj_coupling_tt.  Wtt: float64 CUDA tensor [l3max+1].  Returns TT [(lmax+1),(lmax+1)]."""
+    import torch
+    N = tables.lmax + 1
+    if TT is None:
+        TT = torch.empty((N, N), dtype=torch.float64, device=Wtt.device)
+    nW = tables.l3max + 1
+    _check(load_library().tj_coupling_tt(tables.handle, _dev_ptr(Wtt, nW, "Wtt"), nW, _dev_ptr(TT, N * N, "TT"),
+                                         _stream_ptr(stream)), "tj_coupling_tt")
+    return TT
+
+
+_BLOCKS = ("TT", "TE", "EE", "BB", "EB")
+
+
+def coupling_pol(tables: Tables, Wtt, Wtp, Wpp, want=_BLOCKS, out=None, stream=None):
+    """tj_coupling_pol.  `want`: which blocks to compute; `out`: optional dict of preallocated
+    [(lmax+1),(lmax+1)] float64 CUDA tensors.  Returns dict name -> tensor."""
+    import torch
+    N = tables.lmax + 1
+    nW = tables.l3max + 1
+    dev = next(w for w in (Wtt, Wtp, Wpp) if w is not None).device
+    out = {} if out is None else dict(out)
+    for k in want:
+        if k not in out:
+            out[k] = torch.empty((N, N), dtype=torch.float64, device=dev)
+    args = [_dev_ptr(out.get(k) if k in want else None, N * N, k) for k in _BLOCKS]
+    _check(load_library().tj_coupling_pol(tables.handle, _dev_ptr(Wtt, nW, "Wtt"), _dev_ptr(Wtp, nW, "Wtp"),
+                                          _dev_ptr(Wpp, nW, "Wpp"), nW, *args, _stream_ptr(stream)), "tj_coupling_pol")
+    return {k: out[k] for k in want}
+
+
+def coupling_band(tables: Tables, lcut: int, Wtt, Wtp, Wpp, want=_BLOCKS, out=None, stream=None):
+    """tj_coupling_band.  Windows have lcut+1 entries; outputs are [(lmax+1),(2*lcut+1)] banded."""
+    import torch
+    N = tables.lmax + 1
+    width = 2 * lcut + 1
+    dev = next(w for w in (Wtt, Wtp, Wpp) if w is not None).device
+    out = {} if out is None else dict(out)
+    for k in want:
+        if k not in out:
+            out[k] = torch.empty((N, width), dtype=torch.float64, device=dev)
+    args = [_dev_ptr(out.get(k) if k in want else None, N * width, k) for k in _BLOCKS]
+    _check(load_library().tj_coupling_band(tables.handle, int(lcut), _dev_ptr(Wtt, lcut + 1, "Wtt"),
+                                           _dev_ptr(Wtp, lcut + 1, "Wtp"), _dev_ptr(Wpp, lcut + 1, "Wpp"),
+                                           *args, _stream_ptr(stream)), "tj_coupling_band")
+    return {k: out[k] for k in want}
+
+
+def coupling_host(tables: Tables, Wtt, Wtp, Wpp, out: dict, band_lcut: int | None = None, stream=None):
+    """tj_coupling_host: HOST tensors in, HOST tensors out (`out`: dict name -> preallocated CPU
+    float64 tensor, ideally pinned).  Synchronises before returning."""
+    N = tables.lmax + 1
+    if band_lcut is None:
+        band, n, nw, per = 0, tables.l3max + 1, tables.l3max + 1, N * N
+    else:
+        band, n, nw, per = 1, int(band_lcut), int(band_lcut) + 1, N * (2 * int(band_lcut) + 1)
+    args = [_host_ptr(out.get(k), per, k) for k in _BLOCKS]
+    _check(load_library().tj_coupling_host(tables.handle, band, n, _host_ptr(Wtt, nw, "Wtt"), _host_ptr(Wtp, nw, "Wtp"),
+                                           _host_ptr(Wpp, nw, "Wpp"), *args, _stream_ptr(stream)), "tj_coupling_host")
+    return out
+
+
+def l3_range(l1, l2, l3max, parity):
+    lo, hi, n = ctypes.c_int(), ctypes.c_int(), ctypes.c_int()
+    _check(load_library().tj_l3_range(l1, l2, l3max, parity, ctypes.byref(lo), ctypes.byref(hi), ctypes.byref(n)),
+           "tj_l3_range")
+    return lo.value, hi.value, n.value
+
+
+def sweep_counts(l1, l2, l3max):
+    a, b, c, d = (ctypes.c_int() for _ in range(4))
+    _check(load_library().tj_sweep_counts(l1, l2, l3max, ctypes.byref(a), ctypes.byref(b), ctypes.byref(c), ctypes.byref(d)),
+           "tj_sweep_counts")
+    return a.value, b.value, c.value, d.value
+
+
+def fp64_probe(iters=20000, stream=None):
+    v = ctypes.c_double()
+    _check(load_library().tj_fp64_probe(int(iters), _stream_ptr(stream), ctypes.byref(v)), "tj_fp64_probe")
+    return v.value
+
+
+def launches_per_call(which: int) -> int:
+    return int(load_library().tj_launches_per_call(which))
