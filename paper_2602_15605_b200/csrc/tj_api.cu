@@ -1,0 +1,372 @@
+// tj_api.cu -- the C ABI of libtj (include/tj.h): argument checks, stream-ordered scratch, launches.
+#include <math.h>
+#include <mutex>
+#include <new>
+#include <stdio.h>
+#include <string.h>
+
+#include "tj_internal.cuh"
+
+using namespace tj;
+
+namespace {
+
+thread_local char g_errbuf[256] = "CUDA error";
+
+int cuda_fail(cudaError_t e, const char *where)
+{
+    snprintf(g_errbuf, sizeof(g_errbuf), "CUDA error in %s: %s", where, cudaGetErrorString(e));
+    return e == cudaErrorMemoryAllocation ? TJ_ENOMEM : TJ_ECUDA;
+}
+#define TJ_CUDA(call, where)                                   \
+    do {                                                       \
+        cudaError_t e__ = (call);                              \
+        if (e__ != cudaSuccess) return cuda_fail(e__, where);  \
+    } while (0)
+
+// keep freed scratch in the default mem pool instead of returning it to the OS after every call
+void tune_pool_once()
+{
+    static std::once_flag once;
+    std::call_once(once, [] {
+        int dev = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess) return;
+        cudaMemPool_t pool;
+        if (cudaDeviceGetDefaultMemPool(&pool, dev) != cudaSuccess) return;
+        unsigned long long thr = ~0ull;
+        cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &thr);
+    });
+}
+
+int total_tiles(int lmax, int l3max, int R, bool banded)
+{
+    long long n = 0;
+    const int nb = num_bands(lmax, R);
+    for (int b = 0; b < nb; ++b) n += band_num_tiles(lmax, l3max, R, b, banded);
+    return n > 0x7fffffffLL ? -1 : (int)n;
+}
+
+// One coupling call on device pointers.  lcut < 0: dense (l3max = handle's); else banded with l3 <= lcut.
+int run_coupling(const tj_tables *tables, int lcut, const double *d_Wtt, const double *d_Wtp, const double *d_Wpp,
+                 int nW, double *d_TT, double *d_TE, double *d_EE, double *d_BB, double *d_EB, cudaStream_t st);
+
+}  // namespace
+
+struct tj_tables {
+    Tables T;
+};
+
+extern "C" {
+
+const char *tj_strerror(int code)
+{
+    switch (code) {
+        case TJ_OK: return "ok";
+        case TJ_EINVAL: return "invalid argument";
+        case TJ_ENOMEM: return "out of memory";
+        case TJ_ECUDA: return g_errbuf;
+        default: return "unknown error code";
+    }
+}
+
+int tj_build_tables(int lmax, int l3max, void *cuda_stream, tj_tables **out)
+{
+    if (!out) return TJ_EINVAL;
+    *out = nullptr;
+    if (lmax < 0 || l3max < 0 || lmax > 0x0fffffff / 4 || l3max > 2 * lmax) return TJ_EINVAL;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    tj_tables *h = new (std::nothrow) tj_tables;
+    if (!h) return TJ_ENOMEM;
+    Tables &T = h->T;
+    T.lmax = lmax;
+    T.l3max = l3max;
+    T.pmax = 2 * lmax + 1;
+    T.np_alloc = GUARD_LO + T.pmax + 1 + GUARD_HI;
+    T.nl_alloc = GUARD_LO + 2 * lmax + 1 + GUARD_HI;
+    size_t n = (size_t)5 * T.np_alloc + (size_t)2 * T.nl_alloc;
+    cudaError_t e = cudaMalloc((void **)&T.base, n * sizeof(double));
+    if (e != cudaSuccess) { delete h; return cuda_fail(e, "tj_build_tables/cudaMalloc"); }
+    double *p = T.base + GUARD_LO;
+    T.g = p;    p += T.np_alloc;
+    T.ginv = p; p += T.np_alloc;
+    T.h = p;    p += T.np_alloc;
+    T.gA = p;   p += T.np_alloc;
+    T.gB = p;   p += T.np_alloc;
+    T.u3 = p;   p += T.nl_alloc;
+    T.isd = p;
+    e = launch_build_tables(T, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) { cudaFree(T.base); delete h; return cuda_fail(e, "tj_build_tables"); }
+    tune_pool_once();
+    *out = h;
+    return TJ_OK;
+}
+
+void tj_free_tables(tj_tables *tables)
+{
+    if (!tables) return;
+    cudaFree(tables->T.base);
+    delete tables;
+}
+
+int tj_tables_info(const tj_tables *tables, int *lmax, int *l3max, int *pmax)
+{
+    if (!tables) return TJ_EINVAL;
+    if (lmax) *lmax = tables->T.lmax;
+    if (l3max) *l3max = tables->T.l3max;
+    if (pmax) *pmax = tables->T.pmax;
+    return TJ_OK;
+}
+
+int tj_tables_copy(const tj_tables *tables, int which, double *h_dst, int count)
+{
+    if (!tables || !h_dst || count < 0) return TJ_EINVAL;
+    const Tables &T = tables->T;
+    const double *src = nullptr;
+    int maxn = 0;
+    switch (which) {
+        case 0: src = T.g; maxn = T.pmax + 1; break;
+        case 1: src = T.ginv; maxn = T.pmax + 1; break;
+        case 2: src = T.h; maxn = T.pmax + 1; break;
+        case 3: src = T.gA; maxn = T.pmax + 1; break;
+        case 4: src = T.gB; maxn = T.pmax + 1; break;
+        case 5: src = T.u3; maxn = T.lmax + 1; break;
+        case 6: src = T.isd; maxn = T.lmax + 1; break;
+        default: return TJ_EINVAL;
+    }
+    if (count > maxn) return TJ_EINVAL;
+    TJ_CUDA(cudaMemcpy(h_dst, src, sizeof(double) * (size_t)count, cudaMemcpyDeviceToHost), "tj_tables_copy");
+    return TJ_OK;
+}
+
+int tj_coupling_tt(const tj_tables *tables, const double *d_Wtt, int nW, double *d_TT, void *cuda_stream)
+{
+    if (!tables || !d_Wtt || !d_TT) return TJ_EINVAL;
+    if (nW != tables->T.l3max + 1) return TJ_EINVAL;
+    return run_coupling(tables, -1, d_Wtt, nullptr, nullptr, nW, d_TT, nullptr, nullptr, nullptr, nullptr,
+                        (cudaStream_t)cuda_stream);
+}
+
+int tj_coupling_pol(const tj_tables *tables, const double *d_Wtt, const double *d_Wtp, const double *d_Wpp, int nW,
+                    double *d_TT, double *d_TE, double *d_EE, double *d_BB, double *d_EB, void *cuda_stream)
+{
+    if (!tables) return TJ_EINVAL;
+    if (nW != tables->T.l3max + 1) return TJ_EINVAL;
+    return run_coupling(tables, -1, d_Wtt, d_Wtp, d_Wpp, nW, d_TT, d_TE, d_EE, d_BB, d_EB, (cudaStream_t)cuda_stream);
+}
+
+int tj_coupling_band(const tj_tables *tables, int lcut, const double *d_Wtt, const double *d_Wtp, const double *d_Wpp,
+                     double *d_TT, double *d_TE, double *d_EE, double *d_BB, double *d_EB, void *cuda_stream)
+{
+    if (!tables) return TJ_EINVAL;
+    if (lcut < 0 || lcut > 2 * tables->T.lmax) return TJ_EINVAL;
+    return run_coupling(tables, lcut, d_Wtt, d_Wtp, d_Wpp, lcut + 1, d_TT, d_TE, d_EE, d_BB, d_EB,
+                        (cudaStream_t)cuda_stream);
+}
+
+int tj_coupling_host(const tj_tables *tables, int band, int nW_or_lcut, const double *h_Wtt, const double *h_Wtp,
+                     const double *h_Wpp, double *h_TT, double *h_TE, double *h_EE, double *h_BB, double *h_EB,
+                     void *cuda_stream)
+{
+    if (!tables || nW_or_lcut < 0) return TJ_EINVAL;
+    const Tables &T = tables->T;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const int lcut = band ? nW_or_lcut : -1;
+    const int nW = band ? nW_or_lcut + 1 : nW_or_lcut;
+    if (!band && nW != T.l3max + 1) return TJ_EINVAL;
+    if (band && lcut > 2 * T.lmax) return TJ_EINVAL;
+    const size_t N = (size_t)T.lmax + 1;
+    const size_t per = band ? N * (size_t)(2 * lcut + 1) : N * N;
+    const double *hw[3] = {h_Wtt, h_Wtp, h_Wpp};
+    double *ho[5] = {h_TT, h_TE, h_EE, h_BB, h_EB};
+    // BB is a copy of EE: when both are requested compute one matrix and copy it out twice
+    const bool bb_from_ee = (h_EE && h_BB);
+    int nout = 0;
+    for (int k = 0; k < 5; ++k) if (ho[k] && !(k == 3 && bb_from_ee)) ++nout;
+    if (nout == 0) return TJ_EINVAL;
+    tune_pool_once();
+    double *dw = nullptr, *dout = nullptr;
+    TJ_CUDA(cudaMallocAsync((void **)&dw, sizeof(double) * 3 * (size_t)nW, st), "tj_coupling_host/alloc windows");
+    cudaError_t e = cudaMallocAsync((void **)&dout, sizeof(double) * per * (size_t)nout, st);
+    if (e != cudaSuccess) { cudaFreeAsync(dw, st); return cuda_fail(e, "tj_coupling_host/alloc outputs"); }
+    const double *dwp[3] = {nullptr, nullptr, nullptr};
+    for (int k = 0; k < 3; ++k) {
+        if (!hw[k]) continue;
+        dwp[k] = dw + (size_t)k * nW;
+        e = cudaMemcpyAsync((void *)dwp[k], hw[k], sizeof(double) * (size_t)nW, cudaMemcpyHostToDevice, st);
+        if (e != cudaSuccess) break;
+    }
+    double *dop[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+    int rc = TJ_OK;
+    if (e == cudaSuccess) {
+        int j = 0;
+        for (int k = 0; k < 5; ++k)
+            if (ho[k] && !(k == 3 && bb_from_ee)) dop[k] = dout + per * (size_t)(j++);
+        rc = run_coupling(tables, lcut, dwp[0], dwp[1], dwp[2], nW, dop[0], dop[1], dop[2], dop[3], dop[4], st);
+        if (rc == TJ_OK) {
+            for (int k = 0; k < 5 && e == cudaSuccess; ++k) {
+                const double *src = (k == 3 && bb_from_ee) ? dop[2] : dop[k];
+                if (ho[k]) e = cudaMemcpyAsync(ho[k], src, sizeof(double) * per, cudaMemcpyDeviceToHost, st);
+            }
+        }
+    }
+    cudaFreeAsync(dout, st);
+    cudaFreeAsync(dw, st);
+    cudaError_t es = cudaStreamSynchronize(st);
+    if (rc != TJ_OK) return rc;
+    if (e != cudaSuccess) return cuda_fail(e, "tj_coupling_host/copies");
+    if (es != cudaSuccess) return cuda_fail(es, "tj_coupling_host/sync");
+    return TJ_OK;
+}
+
+int tj_l3_range(int l1, int l2, int l3max, int parity, int *l3_lo, int *l3_hi, int *nterms)
+{
+    if (l1 < 0 || l2 < 0 || l3max < 0 || (parity != 0 && parity != 1)) return TJ_EINVAL;
+    // expressed through the step indices the kernel walks (tj_sweep_counts): l3 = s-2t-parity
+    int te_lo, te_hi, to_lo, to_hi;
+    tj_sweep_counts(l1, l2, l3max, &te_lo, &te_hi, &to_lo, &to_hi);
+    const int s = l1 + l2;
+    const int t_lo = parity ? to_lo : te_lo, t_hi = parity ? to_hi : te_hi;
+    int n = t_hi - t_lo + 1;
+    int lo = s - 2 * t_hi - parity, hi = s - 2 * t_lo - parity;
+    if (n <= 0) { n = 0; hi = lo - 2; }   // empty: hi < lo
+    if (l3_lo) *l3_lo = lo;
+    if (l3_hi) *l3_hi = hi;
+    if (nterms) *nterms = n;
+    return TJ_OK;
+}
+
+int tj_sweep_counts(int l1, int l2, int l3max, int *te_lo, int *te_hi, int *to_lo, int *to_hi)
+{
+    if (l1 < 0 || l2 < 0 || l3max < 0) return TJ_EINVAL;
+    const int s = l1 + l2, mn = l1 < l2 ? l1 : l2;
+    int a = s - l3max;          // even: s-2t <= l3max
+    a = a > 0 ? (a + 1) >> 1 : 0;
+    int b = s - 1 - l3max;      // odd:  s-2t-1 <= l3max
+    b = b > 0 ? (b + 1) >> 1 : 0;
+    if (te_lo) *te_lo = a;
+    if (te_hi) *te_hi = mn;
+    if (to_lo) *to_lo = b;
+    if (to_hi) *to_hi = mn - 1;
+    return TJ_OK;
+}
+
+int tj_fp64_probe(int iters, void *cuda_stream, double *h_thread_instr_per_s)
+{
+    if (iters <= 0 || !h_thread_instr_per_s) return TJ_EINVAL;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int dev = 0, sms = 0;
+    TJ_CUDA(cudaGetDevice(&dev), "tj_fp64_probe");
+    TJ_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev), "tj_fp64_probe");
+    const int threads = 256, blocks = sms * 4;
+    double *sink = nullptr;
+    TJ_CUDA(cudaMalloc((void **)&sink, sizeof(double) * (size_t)blocks * threads), "tj_fp64_probe/alloc");
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0);
+    cudaEventCreate(&e1);
+    cudaError_t e = launch_fp64_probe(iters / 8 + 1, sink, blocks, threads, st);  // warm-up
+    cudaEventRecord(e0, st);
+    if (e == cudaSuccess) e = launch_fp64_probe(iters, sink, blocks, threads, st);
+    cudaEventRecord(e1, st);
+    cudaError_t es = cudaEventSynchronize(e1);
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, e0, e1);
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(sink);
+    if (e != cudaSuccess) return cuda_fail(e, "tj_fp64_probe/launch");
+    if (es != cudaSuccess) return cuda_fail(es, "tj_fp64_probe/sync");
+    // 16 DFMA per loop iteration per thread
+    const double instr = 16.0 * (double)iters * (double)blocks * (double)threads;
+    *h_thread_instr_per_s = instr / ((double)ms * 1e-3);
+    return TJ_OK;
+}
+
+int tj_launches_per_call(int which)
+{
+    // prepare + sweep + writer; the band call adds no kernel (its zero-fill is a memset)
+    return (which >= 0 && which <= 2) ? 3 : TJ_EINVAL;
+}
+
+}  // extern "C"
+
+namespace {
+
+int run_coupling(const tj_tables *tables, int lcut, const double *d_Wtt, const double *d_Wtp, const double *d_Wpp,
+                 int nW, double *d_TT, double *d_TE, double *d_EE, double *d_BB, double *d_EB, cudaStream_t st)
+{
+    const Tables &T = tables->T;
+    const bool banded = lcut >= 0;
+    // an output needs its window (TJ_EINVAL otherwise)
+    if ((d_TT && !d_Wtt) || (d_TE && !d_Wtp) || ((d_EE || d_BB || d_EB) && !d_Wpp)) return TJ_EINVAL;
+    if (!d_TT && !d_TE && !d_EE && !d_BB && !d_EB) return TJ_EINVAL;
+    // EE target: EE if given, else BB takes the even spin-2 block directly
+    double *ee = d_EE ? d_EE : d_BB;
+    double *bb_copy = (d_EE && d_BB) ? d_BB : nullptr;
+
+    // smallest instantiated sweep that covers the request
+    int mask;
+    if (!d_TE && !ee && !d_EB) mask = M_TT;
+    else if (d_TT) mask = M_TT | M_TE | M_EE | M_EB;
+    else mask = M_TE | M_EE | M_EB;
+    const int R = (mask == M_TT) ? R_TT : R_POL;
+    const int l3max_eff = banded ? lcut : T.l3max;
+    const long long N = (long long)T.lmax + 1;
+    const long long ld = banded ? (long long)(2 * lcut + 1) : N;
+    const size_t per = (size_t)N * (size_t)ld;
+
+    const int ntiles = total_tiles(T.lmax, l3max_eff, R, banded);
+    if (ntiles < 0) return TJ_EINVAL;
+    const int nb = num_bands(T.lmax, R);
+
+    // ---- stream-ordered scratch: 3 prefolded windows + tile prefix
+    const size_t wbytes = sizeof(double) * 3 * (size_t)T.nl_alloc;
+    const size_t tbytes = sizeof(int) * (size_t)(nb + 1 + 1);
+    const size_t tb_al = (tbytes + 15) & ~(size_t)15;
+    unsigned char *scratch = nullptr;
+    TJ_CUDA(cudaMallocAsync((void **)&scratch, wbytes + tb_al, st), "coupling/scratch");
+    double *wtt = (double *)scratch + GUARD_LO;
+    double *wtp = wtt + T.nl_alloc;
+    double *wpp = wtp + T.nl_alloc;
+    int *tile_start = (int *)(scratch + wbytes);
+
+    int rc = TJ_OK;
+    cudaError_t e = launch_prepare(T, d_Wtt, d_Wtp, d_Wpp, nW, wtt, wtp, wpp, tile_start, R, l3max_eff, banded, st);
+    if (e == cudaSuccess && banded) {
+        // slots of the band whose l2 falls outside 0..lmax (and everything the sweep does not own) are 0
+        double *outs[5] = {d_TT, d_TE, d_EE, d_BB, d_EB};
+        for (int k = 0; k < 5 && e == cudaSuccess; ++k)
+            if (outs[k]) e = cudaMemsetAsync(outs[k], 0, sizeof(double) * per, st);
+    }
+    if (e == cudaSuccess) {
+        SweepParams P;
+        P.g = T.g; P.ginv = T.ginv; P.h = T.h; P.gA = T.gA; P.gB = T.gB; P.u3 = T.u3; P.isd = T.isd;
+        P.wtt = wtt; P.wtp = wtp; P.wpp = wpp;
+        // a block the instantiated sweep computes but the caller did not ask for has a NULL target
+        // and is not stored
+        P.TT = d_TT; P.TE = d_TE; P.EE = ee; P.EB = d_EB;
+        P.tile_start = tile_start;
+        P.lmax = T.lmax; P.l3max = l3max_eff; P.nbands = nb; P.lcut = banded ? lcut : -1; P.ld = ld;
+        e = launch_sweep(P, mask, ntiles, st);
+    }
+    if (e == cudaSuccess) {
+        WriterParams W;
+        memset(&W, 0, sizeof(W));
+        int n = 0;
+        W.bb = nullptr; W.bb_src = -1;
+        if (d_TT) W.M[n++] = d_TT;
+        if (d_TE) W.M[n++] = d_TE;
+        if (ee) { if (bb_copy) { W.bb = bb_copy; W.bb_src = n; } W.M[n++] = ee; }
+        if (d_EB) W.M[n++] = d_EB;
+        W.nmat = n;
+        W.lmax = T.lmax; W.lcut = banded ? lcut : -1; W.ld = ld;
+        W.ntile = (int)((N + 31) / 32);
+        W.tile_band = banded ? ((lcut + 31) / 32 + 1 < W.ntile - 1 ? (lcut + 31) / 32 + 1 : W.ntile - 1) : W.ntile - 1;
+        e = launch_writer(W, st);
+    }
+    if (e != cudaSuccess) rc = cuda_fail(e, "coupling");
+    cudaFreeAsync(scratch, st);
+    return rc;
+}
+
+}  // namespace

@@ -1,0 +1,89 @@
+// tj_internal.cuh -- shared declarations of libtj (not part of the public ABI).
+//
+// Notation follows PAPER.md / DESIGN.md: lmax, l3max, s = l1+l2, step t (even: l3 = s-2t,
+// odd: l3 = s-2t-1), p = J/2, g(p) of Eq. 11, u_l = l(l+1), D_l = (l-1)l(l+1)(l+2).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include "../../include/tj.h"
+
+namespace tj {
+
+// ---- table layout -------------------------------------------------------------------------
+// Every p-indexed table (g, ginv, h, gA, gB) and every l3-indexed array (prefolded windows, u3)
+// is allocated as [GUARD_LO + n + GUARD_HI] doubles and addressed through a pointer to index 0,
+// so out-of-triangle steps read exact zeros instead of branching ("guard bands").
+constexpr int GUARD_LO = 256;
+constexpr int GUARD_HI = 768;
+
+// ---- sweep tile geometry -------------------------------------------------------
+// A thread owns R pairs on ONE anti-diagonal: (l1, l2) = (a+i, c-i), i = 0..R-1, a = band*R.
+// Lanes run along c, so a warp covers rows a..a+R-1 and a skewed window of 32+R-1 columns.
+constexpr int SWEEP_THREADS = 128;   // columns c per CTA
+constexpr int R_POL = 8;             // pairs per thread, fused TT+TE+EE(+EB) sweep
+constexpr int R_TT = 16;             // pairs per thread, TT-only sweep
+
+// mask bits of the blocks one sweep computes
+constexpr int M_TT = 1, M_TE = 2, M_EE = 4, M_EB = 8;
+
+__host__ __device__ inline int num_bands(int lmax, int R) { return (lmax + R) / R; }  // ceil((lmax+1)/R)
+
+// columns c needed by row band `band`: c_lo = a; c_hi as below (inclusive)
+__host__ __device__ inline int band_c_hi(int lmax, int l3max, int R, int band, bool banded)
+{
+    int a = band * R;
+    int hi = lmax + R - 1;
+    if (banded) {
+        long long alt = (long long)a + 2 * R - 2 + l3max;
+        if (alt < hi) hi = (int)alt;
+    }
+    return hi;
+}
+__host__ __device__ inline int band_num_tiles(int lmax, int l3max, int R, int band, bool banded)
+{
+    int a = band * R;
+    int hi = band_c_hi(lmax, l3max, R, band, banded);
+    return hi >= a ? (hi - a + SWEEP_THREADS) / SWEEP_THREADS : 0;
+}
+
+struct Tables {
+    int lmax, l3max, pmax;          // p-tables hold p = 0..pmax = 2*lmax+1
+    int np_alloc;                   // doubles per p-table incl. guards
+    int nl_alloc;                   // doubles per l-table incl. guards (index range -GUARD_LO .. 2*lmax+GUARD_HI)
+    double *base;                   // one device allocation
+    // pointers to index 0
+    double *g, *ginv, *h, *gA, *gB; // p-indexed
+    double *u3;                     // l-indexed: u3[l] = l(l+1)
+    double *isd;                    // l-indexed: 1/sqrt(D_l), 0 for l < 2
+};
+
+struct SweepParams {
+    const double *g, *ginv, *h, *gA, *gB, *u3, *isd;
+    const double *wtt, *wtp, *wpp;  // prefolded windows W'_X[l] = (2l+1) W_X[l] / (4 pi), pointer to l = 0
+    double *TT, *TE, *EE, *EB;      // raw Xi, upper triangle (dense: [l1*ld+l2]; band: [l1*ld + l2-l1+lcut])
+    const int *tile_start;          // [nbands+1] exclusive prefix of tiles per band, bands in DESCENDING order
+    int lmax, l3max, nbands, lcut;  // lcut < 0: dense storage
+    long long ld;                   // row stride of the outputs
+};
+
+struct WriterParams {
+    double *M[5];                   // TT, TE, EE, EB, (BB copy of EE or NULL)
+    int nmat;                       // entries of M that take part in the mirror (<= 4)
+    double *bb;                     // if non-NULL: receives a copy of M[bb_src]
+    int bb_src;
+    int lmax, lcut;                 // lcut < 0: dense
+    long long ld;
+    int ntile;                      // tiles per side (ceil((lmax+1)/32))
+    int tile_band;                  // banded: tiles (I,J) with J-I <= tile_band
+};
+
+// kernels / launchers (defined in the .cu files)
+cudaError_t launch_build_tables(const Tables &T, cudaStream_t st);
+cudaError_t launch_prepare(const Tables &T, const double *d_Wtt, const double *d_Wtp, const double *d_Wpp, int nW,
+                           double *wtt, double *wtp, double *wpp, int *tile_start, int R, int l3max_eff, bool banded,
+                           cudaStream_t st);
+cudaError_t launch_sweep(const SweepParams &P, int mask, int total_tiles, cudaStream_t st);
+cudaError_t launch_writer(const WriterParams &P, cudaStream_t st);
+cudaError_t launch_fp64_probe(int iters, double *d_sink, int blocks, int threads, cudaStream_t st);
+
+}  // namespace tj

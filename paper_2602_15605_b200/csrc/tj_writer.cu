@@ -1,0 +1,82 @@
+// tj_writer.cu -- triangle -> full matrix writer (step a6), dense and banded.
+//
+// The sweep leaves Xi(l1,l2), l1 <= l2, in the upper triangle of each output.  Xi is symmetric
+// (PAPER.md:236 as read in DESIGN.md reading #8) and K_{l1 l2} = (2 l2+1) Xi(l1,l2), so
+//     M[l1][l2] = (2 l2+1) Xi,      M[l2][l1] = (2 l1+1) Xi.
+// One CTA owns one 32x32 tile pair (I,J), I <= J: it reads the Xi tile once (coalesced along l2), scales
+// it in place, and writes the mirrored tile through a shared-memory transpose so that both writes are
+// full coalesced row segments.  Both products use the SAME Xi double, so (2 l1+1) M[l1][l2] and
+// (2 l2+1) M[l2][l1] agree to the last rounding.  BB, when requested next to EE, is written from the
+// same registers.
+//
+// Banded storage (step a7): address(l1,l2) = l1*ld + (l2-l1+lcut), valid for |l1-l2| <= lcut; only tile
+// pairs within the band are launched; slots whose l2 is outside 0..lmax were zeroed by the API.
+#include "tj_internal.cuh"
+
+namespace tj {
+namespace {
+
+constexpr int WT = 32;          // tile edge
+constexpr int WROWS = 8;        // rows per pass (blockDim.y)
+
+__device__ __forceinline__ long long addr(int r, int c, long long ld, int lcut)
+{
+    return lcut < 0 ? (long long)r * ld + c : (long long)r * ld + (c - r + lcut);
+}
+
+__global__ void __launch_bounds__(WT * WROWS) writer_kernel(const __grid_constant__ WriterParams P)
+{
+    __shared__ double tile[WT][WT + 1];
+    // tile pair decode: blockIdx.x enumerates (I, dJ) with J = I + dJ
+    const int I = blockIdx.x / (P.tile_band + 1);
+    const int J = I + blockIdx.x % (P.tile_band + 1);
+    if (J >= P.ntile) return;
+    const int m = blockIdx.y;
+    double *M = P.M[m];
+    double *bb = (P.bb != nullptr && m == P.bb_src) ? P.bb : nullptr;
+    const int tx = threadIdx.x, ty = threadIdx.y;
+    const int N = P.lmax + 1;
+
+    // ---- read Xi tile (rows l1 in I, cols l2 in J), scale in place ----
+    const int l2 = J * WT + tx;
+#pragma unroll
+    for (int k = 0; k < WT; k += WROWS) {
+        const int l1 = I * WT + ty + k;
+        double xi = 0.0;
+        const bool ok = l1 < N && l2 < N && l2 >= l1 && (P.lcut < 0 || l2 - l1 <= P.lcut);
+        if (ok) {
+            const long long ix = addr(l1, l2, P.ld, P.lcut);
+            xi = M[ix];
+            const double v = xi * (double)(2 * l2 + 1);
+            M[ix] = v;
+            if (bb) bb[ix] = v;
+        }
+        tile[ty + k][tx] = xi;
+    }
+    __syncthreads();
+    // ---- mirrored tile: rows r = l2 in J, cols q = l1 in I; strictly lower triangle only ----
+    const int q = I * WT + tx;
+#pragma unroll
+    for (int k = 0; k < WT; k += WROWS) {
+        const int r = J * WT + ty + k;
+        if (r < N && q < N && q < r && (P.lcut < 0 || r - q <= P.lcut)) {
+            const double v = tile[tx][ty + k] * (double)(2 * q + 1);
+            const long long ix = addr(r, q, P.ld, P.lcut);
+            M[ix] = v;
+            if (bb) bb[ix] = v;
+        }
+    }
+}
+
+}  // namespace
+
+cudaError_t launch_writer(const WriterParams &P, cudaStream_t st)
+{
+    if (P.nmat <= 0) return cudaSuccess;
+    dim3 grid((unsigned)(P.ntile * (P.tile_band + 1)), (unsigned)P.nmat, 1);
+    dim3 block(WT, WROWS, 1);
+    writer_kernel<<<grid, block, 0, st>>>(P);
+    return cudaGetLastError();
+}
+
+}  // namespace tj

@@ -1,0 +1,87 @@
+"""The C-ABI library builds, loads and exports every symbol include/tj.h declares (no compute calls:
+this runs without a GPU), and its host-side integer helpers agree with the oracle's bookkeeping."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_2602_15605_b200 import binding, build
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    build.build()
+    return binding.load_library()
+
+
+def _header_symbols():
+    src = open(os.path.join(ROOT, "include", "tj.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(tj_[a-z0-9_]+)\s*\(", src)))
+
+
+def test_every_declared_symbol_is_exported(lib):
+    declared = _header_symbols()
+    assert declared == sorted(binding.SYMBOLS)
+    for name in declared:
+        assert hasattr(lib, name), name
+        assert ctypes.cast(getattr(lib, name), ctypes.c_void_p).value
+
+
+def test_strerror(lib):
+    assert lib.tj_strerror(0) == b"ok"
+    assert b"invalid" in lib.tj_strerror(-1)
+    assert lib.tj_launches_per_call(1) == 3
+
+
+def test_argument_errors_without_gpu(lib):
+    # argument validation happens before any CUDA call
+    h = ctypes.c_void_p()
+    assert lib.tj_build_tables(-1, 0, None, ctypes.byref(h)) == binding.TJ_EINVAL
+    assert lib.tj_build_tables(10, 21, None, ctypes.byref(h)) == binding.TJ_EINVAL
+    assert lib.tj_build_tables(10, 20, None, None) == binding.TJ_EINVAL
+    assert lib.tj_coupling_tt(None, None, 1, None, None) == binding.TJ_EINVAL
+    assert lib.tj_l3_range(-1, 0, 0, 0, None, None, None) == binding.TJ_EINVAL
+    assert lib.tj_l3_range(1, 1, 5, 2, None, None, None) == binding.TJ_EINVAL
+
+
+def test_l3_range_matches_oracle_bookkeeping(lib):
+    """Bit-exact triangle / l3-range bookkeeping (north_star): all pairs of a small case, random
+    pairs at the sizes of the other configs incl. truncated l3max and the band cut."""
+    rng = np.random.default_rng(7)
+    cases = [(l1, l2, 512) for l1 in range(0, 257, 5) for l2 in range(0, 257, 3)]
+    for lmax, l3max in ((2000, 4000), (5000, 10000), (10000, 20000), (15000, 300), (300, 17), (40, 0)):
+        l1 = rng.integers(0, lmax + 1, 4000)
+        l2 = rng.integers(0, lmax + 1, 4000)
+        near = np.clip(l1 + rng.integers(-l3max - 3, l3max + 4, 4000), 0, lmax)
+        cases += [(int(a), int(b), l3max) for a, b in zip(l1, l2)]
+        cases += [(int(a), int(b), l3max) for a, b in zip(l1, near)]
+    for l1, l2, l3max in cases:
+        for parity in (0, 1):
+            o = oracle.l3_range(l1, l2, l3max, parity)
+            g = binding.l3_range(l1, l2, l3max, parity)
+            assert o[2] == g[2], (l1, l2, l3max, parity, o, g)
+            if o[2] > 0:
+                assert o == g, (l1, l2, l3max, parity, o, g)
+            else:
+                assert g[0] > g[1]
+        te_lo, te_hi, to_lo, to_hi = binding.sweep_counts(l1, l2, l3max)
+        s = l1 + l2
+        even = [s - 2 * t for t in range(te_lo, te_hi + 1)]
+        odd = [s - 2 * t - 1 for t in range(to_lo, to_hi + 1)]
+        lo, hi, n = oracle.l3_range(l1, l2, l3max, 0)
+        assert len(even) == n and (n == 0 or (min(even), max(even)) == (lo, hi))
+        lo, hi, n = oracle.l3_range(l1, l2, l3max, 1)
+        assert len(odd) == n and (n == 0 or (min(odd), max(odd)) == (lo, hi))
+
+
+def test_binding_fails_loudly_without_library(monkeypatch, tmp_path):
+    monkeypatch.setattr(binding, "_LIB", None)
+    monkeypatch.setattr(binding, "_SO", str(tmp_path / "nope.so"))
+    with pytest.raises(binding.TJError):
+        binding.load_library()

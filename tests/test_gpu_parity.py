@@ -1,0 +1,357 @@
+"""Parity of the CUDA path (through the C ABI) against the oracle.  All tests need a B200: -m gpu.
+
+Bar (north_star), element-wise:
+    |gpu - oracle| <= 1e-10 |oracle|   where |oracle| >= 1e-4,
+    |gpu - oracle| <= 1e-14            elsewhere,
+and exact structure: entries the triangle / parity / l3max rules make empty are exactly 0.0.
+"""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_2602_15605_b200 import binding, build, windows
+
+pytestmark = pytest.mark.gpu
+
+RTOL, ATOL_SMALL, SMALL = 1e-10, 1e-14, 1e-4
+BLOCKS = ("TT", "TE", "EE", "BB", "EB")
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _lib():
+    build.build()
+    binding.load_library()
+
+
+def _t(a):
+    import torch
+    return None if a is None else torch.as_tensor(np.ascontiguousarray(a), dtype=torch.float64).cuda()
+
+
+def assert_parity(gpu, ref, what):
+    gpu = np.asarray(gpu, dtype=np.float64)
+    ref = np.asarray(ref, dtype=np.float64)
+    assert gpu.shape == ref.shape, what
+    assert np.all(np.isfinite(gpu)), what
+    err = np.abs(gpu - ref)
+    big = np.abs(ref) >= SMALL
+    bad_big = big & (err > RTOL * np.abs(ref))
+    bad_small = (~big) & (err > ATOL_SMALL)
+    if bad_big.any() or bad_small.any():
+        i = np.argwhere(bad_big | bad_small)[0]
+        raise AssertionError("%s: %d entries out of tolerance, first at %s: gpu=%r oracle=%r" % (
+            what, int(bad_big.sum() + bad_small.sum()), tuple(i), gpu[tuple(i)], ref[tuple(i)]))
+    rel = err[big] / np.abs(ref[big]) if big.any() else np.zeros(1)
+    return float(rel.max()), float(err[~big].max()) if (~big).any() else 0.0
+
+
+def run_pol(lmax, l3max, Wtt, Wtp, Wpp, want=BLOCKS):
+    T = binding.build_tables(lmax, l3max)
+    out = binding.coupling_pol(T, _t(Wtt), _t(Wtp), _t(Wpp), want=want)
+    import torch
+    torch.cuda.synchronize()
+    res = {k: v.cpu().numpy() for k, v in out.items()}
+    T.close()
+    return res
+
+
+# ---------------------------------------------------------------- T1 tables
+def test_tables_against_exact_definition():
+    lmax = 10000
+    T = binding.build_tables(lmax)
+    assert T.pmax == 2 * lmax + 1
+    ref = oracle.table_entries_float(T.pmax)
+    for which, name in enumerate(("g", "ginv", "h", "gA", "gB")):
+        got = T.copy_table(which, T.pmax + 1)
+        ulp = np.spacing(np.abs(ref[name]))
+        d = np.abs(got - ref[name])
+        assert np.all(d <= ulp), (name, int(np.argmax(d / np.maximum(ulp, 1e-300))))
+        # faithfully rounded: the overwhelming majority is bit-identical to the correctly rounded value
+        assert np.mean(got == ref[name]) > 0.99, name
+    g = T.copy_table(0, 4)
+    assert list(g[:3]) == [1.0, 0.5, 0.375]          # g(0), g(1), g(2)  (Eq. 11)
+    p = np.arange(1, T.pmax + 1)
+    gg = T.copy_table(0, T.pmax + 1)[1:]
+    assert abs(gg[-1] * math.sqrt(math.pi * p[-1]) - 1.0) < 1e-4   # g ~ (pi p)^(-1/2)
+    u = T.copy_table(5, lmax + 1)
+    assert np.array_equal(u, np.arange(lmax + 1.0) * (np.arange(lmax + 1.0) + 1.0))
+    isd = T.copy_table(6, lmax + 1)
+    l = np.arange(2, lmax + 1, dtype=np.float64)
+    np.testing.assert_allclose(isd[2:], 1.0 / np.sqrt((l - 1) * l * (l + 1) * (l + 2)), rtol=4e-16)
+    assert isd[0] == 0 and isd[1] == 0
+    T.close()
+
+
+# ---------------------------------------------------------------- T3 configs, full
+def test_cfg0_tt_lmax256_full():
+    wl = windows.config(0)
+    T = binding.build_tables(wl.lmax)
+    TT = binding.coupling_tt(T, _t(wl.Wtt)).cpu().numpy()
+    ref = oracle.coupling_full(wl.lmax, wl.l3max, wl.Wtt, None, None)["TT"]
+    assert TT.shape == (257, 257)
+    assert_parity(TT, ref, "cfg0 TT")
+    # the fused pol sweep must give the same TT
+    both = binding.coupling_pol(T, _t(wl.Wtt), _t(wl.Wtt), _t(wl.Wtt))
+    assert_parity(both["TT"].cpu().numpy(), ref, "cfg0 TT via pol")
+    T.close()
+
+
+def test_cfg0b_full_sky_identity_exact_structure():
+    lmax = 256
+    W = windows.full_sky(2 * lmax)
+    K = run_pol(lmax, 2 * lmax, W, W, W)
+    N = lmax + 1
+    off = ~np.eye(N, dtype=bool)
+    for k in BLOCKS:
+        assert np.all(K[k][off] == 0.0), k
+    np.testing.assert_allclose(np.diag(K["TT"]), 1.0, rtol=1e-14)
+    for k in ("TE", "EE", "BB"):
+        np.testing.assert_allclose(np.diag(K[k])[2:], 1.0, rtol=1e-14)
+        assert np.all(np.diag(K[k])[:2] == 0.0)
+    assert np.all(K["EB"] == 0.0)
+    T = binding.build_tables(lmax)
+    TT = binding.coupling_tt(T, _t(W)).cpu().numpy()
+    assert np.all(TT[off] == 0.0)
+    np.testing.assert_allclose(np.diag(TT), 1.0, rtol=1e-14)
+    T.close()
+
+
+def test_flat_window_closed_form_lmax700():
+    """W = 1: TT = (2 l2+1)/4pi, TE = 0, EE+EB = (2 l2+1)/4pi -- exercises every (l1,l2,l3) term,
+    no oracle needed (closed form)."""
+    lmax = 700
+    W = windows.flat(2 * lmax)
+    K = run_pol(lmax, 2 * lmax, W, W, W)
+    N = lmax + 1
+    expect = np.broadcast_to((2.0 * np.arange(N) + 1.0) / (4 * math.pi), (N, N))
+    np.testing.assert_allclose(K["TT"], expect, rtol=1e-12)
+    assert np.max(np.abs(K["TE"])) < 1e-11
+    np.testing.assert_allclose((K["EE"] + K["EB"])[2:, 2:], expect[2:, 2:], rtol=1e-12)
+    for k in ("TE", "EE", "BB", "EB"):
+        assert np.all(K[k][:2] == 0.0) and np.all(K[k][:, :2] == 0.0)
+
+
+def test_cfg1_recipe_lmax300_full_all_blocks():
+    wl = windows.config(1, lmax=300)   # several CTAs per band, ragged tail (301 = 2*128 + 45)
+    K = run_pol(wl.lmax, wl.l3max, wl.Wtt, wl.Wtp, wl.Wpp)
+    ref = oracle.coupling_full(wl.lmax, wl.l3max, wl.Wtt, wl.Wtp, wl.Wpp)
+    for k in BLOCKS:
+        assert_parity(K[k], ref[k], "cfg1@300 " + k)
+    assert np.array_equal(K["BB"], K["EE"])
+
+
+@pytest.mark.parametrize("lmax", [0, 1, 2, 3, 7, 8, 15, 16, 17, 31, 127, 128, 129])
+def test_ragged_and_tiny_sizes(lmax):
+    wl = windows.config(2, lmax=lmax)
+    K = run_pol(wl.lmax, wl.l3max, wl.Wtt, wl.Wtp, wl.Wpp)
+    ref = oracle.coupling_full(wl.lmax, wl.l3max, wl.Wtt, wl.Wtp, wl.Wpp)
+    for k in BLOCKS:
+        assert K[k].shape == (lmax + 1, lmax + 1)
+        assert_parity(K[k], ref[k], "lmax=%d %s" % (lmax, k))
+    T = binding.build_tables(lmax)
+    TT = binding.coupling_tt(T, _t(wl.Wtt)).cpu().numpy()
+    assert_parity(TT, ref["TT"], "lmax=%d TT-only" % lmax)
+    T.close()
+
+
+def test_truncated_l3max_and_signed_window():
+    lmax, l3max = 200, 137
+    rng = np.random.default_rng(9)
+    W = [rng.standard_normal(l3max + 1) for _ in range(3)]    # signed: TE/EE sums cancel
+    K = run_pol(lmax, l3max, *W)
+    ref = oracle.coupling_full(lmax, l3max, *W)
+    for k in BLOCKS:
+        # tolerance relative to the row scale for signed sums: the bar's absolute branch
+        assert_parity(K[k], ref[k], "l3max<2lmax " + k)
+        i, j = np.indices(K[k].shape)
+        assert np.all(K[k][np.abs(i - j) > l3max] == 0.0)
+
+
+# ---------------------------------------------------------------- T2 spikes: one symbol per entry, exact zero pattern
+@pytest.mark.parametrize("L", [0, 1, 2, 3, 64, 199, 200, 399, 400])
+def test_spike_window_structure_bit_exact(L):
+    lmax = 200
+    W = windows.spike(2 * lmax, L)
+    K = run_pol(lmax, 2 * lmax, W, W, W)
+    ref = oracle.coupling_full(lmax, 2 * lmax, W, W, W)
+    l1, l2 = np.indices((lmax + 1, lmax + 1))
+    inside = (np.abs(l1 - l2) <= L) & (L <= l1 + l2)
+    even = ((l1 + l2 + L) % 2) == 0
+    pol = (l1 >= 2) & (l2 >= 2)
+    # bookkeeping: the zero pattern is fixed by triangle + parity; must hold EXACTLY on the GPU
+    assert np.all(K["TT"][~(inside & even)] == 0.0)
+    assert np.all(K["TT"][inside & even] > 0.0)
+    assert np.all(K["EE"][~(inside & even & pol)] == 0.0)
+    assert np.all(K["TE"][~(inside & even & pol)] == 0.0)
+    assert np.all(K["EB"][~(inside & ~even & pol)] == 0.0)
+    for k in BLOCKS:
+        assert_parity(K[k], ref[k], "spike L=%d %s" % (L, k))
+
+
+# ---------------------------------------------------------------- symmetry / mirror
+def test_mirror_symmetry_bitwise():
+    wl = windows.config(1, lmax=333)
+    K = run_pol(wl.lmax, wl.l3max, wl.Wtt, wl.Wtp, wl.Wpp)
+    w = 2.0 * np.arange(wl.lmax + 1) + 1.0
+    for k in BLOCKS:
+        M = K[k]
+        a = M * w[:, None]          # (2 l1+1) M[l1][l2]
+        b = (M * w[:, None]).T      # (2 l2+1) M[l2][l1]
+        # both sides are (2l1+1)(2l2+1) Xi with one rounding each of the inner product: <= 1 ulp apart
+        assert np.all(np.abs(a - b) <= np.spacing(np.maximum(np.abs(a), np.abs(b)))), k
+
+
+# ---------------------------------------------------------------- nullable outputs
+def test_nullable_outputs_and_errors():
+    wl = windows.config(1, lmax=150)
+    ref = run_pol(wl.lmax, wl.l3max, wl.Wtt, wl.Wtp, wl.Wpp)
+    for want in (("TT",), ("EE",), ("BB",), ("EB",), ("TE",), ("TE", "EB"), ("TT", "BB"), ("EE", "BB", "EB")):
+        got = run_pol(wl.lmax, wl.l3max,
+                      wl.Wtt if "TT" in want else None,
+                      wl.Wtp if "TE" in want else None,
+                      wl.Wpp if set(want) & {"EE", "BB", "EB"} else None, want=want)
+        assert set(got) == set(want)
+        for k in want:
+            assert np.array_equal(got[k], ref[k]), (want, k)
+    T = binding.build_tables(wl.lmax)
+    with pytest.raises(binding.TJError):   # output without its window
+        binding.coupling_pol(T, None, _t(wl.Wtp), _t(wl.Wpp), want=("TT",))
+    with pytest.raises(binding.TJError):   # wrong window length
+        binding.coupling_tt(T, _t(wl.Wtt[:-1]))
+    T.close()
+
+
+# ---------------------------------------------------------------- band variant
+@pytest.mark.parametrize("lmax,lcut", [(400, 30), (257, 0), (100, 150), (64, 7), (300, 300)])
+def test_band_equals_oracle_and_zero_padded_full(lmax, lcut):
+    import torch
+    wl = windows.config(4, lmax=max(lmax, 10))
+    W = np.zeros(lcut + 1)
+    n = min(lcut + 1, wl.Wtt.size)
+    W[:n] = wl.Wtt[:n]
+    T = binding.build_tables(lmax)
+    out = binding.coupling_band(T, lcut, _t(W), _t(W), _t(W))
+    torch.cuda.synchronize()
+    band = {k: v.cpu().numpy() for k, v in out.items()}
+    ref = oracle.coupling_band(lmax, lcut, W, W, W)
+    for k in BLOCKS:
+        assert band[k].shape == (lmax + 1, 2 * lcut + 1)
+        assert_parity(band[k], ref[k], "band %s" % k)
+    # band == dense call with the zero-padded window, on the band; dense is zero outside
+    Wpad = np.zeros(2 * lmax + 1)
+    m = min(lcut + 1, 2 * lmax + 1)
+    Wpad[:m] = W[:m]
+    full = binding.coupling_pol(T, _t(Wpad), _t(Wpad), _t(Wpad))
+    torch.cuda.synchronize()
+    for k in BLOCKS:
+        F = full[k].cpu().numpy()
+        i, j = np.indices(F.shape)
+        assert np.all(F[np.abs(i - j) > lcut] == 0.0)
+        for o in range(-lcut, lcut + 1):
+            rows = np.arange(max(0, -o), min(lmax, lmax - o) + 1)
+            if rows.size:
+                assert np.array_equal(band[k][rows, o + lcut], F[rows, rows + o]), (k, o)
+        # out-of-range slots are zero
+        for l1 in (0, 1, lmax):
+            for o in range(-lcut, lcut + 1):
+                if not (0 <= l1 + o <= lmax):
+                    assert band[k][l1, o + lcut] == 0.0
+    T.close()
+
+
+# ---------------------------------------------------------------- host-buffer (end-to-end) entry point
+def test_host_entry_point_matches_device_path():
+    import torch
+    wl = windows.config(1, lmax=200)
+    ref = run_pol(wl.lmax, wl.l3max, wl.Wtt, wl.Wtp, wl.Wpp)
+    T = binding.build_tables(wl.lmax)
+    N = wl.lmax + 1
+    out = {k: torch.empty((N, N), dtype=torch.float64).pin_memory() for k in BLOCKS}
+    hw = [torch.as_tensor(w).pin_memory() for w in (wl.Wtt, wl.Wtp, wl.Wpp)]
+    binding.coupling_host(T, *hw, out)
+    for k in BLOCKS:
+        assert np.array_equal(out[k].numpy(), ref[k]), k
+    # banded host form
+    lcut = 20
+    W = torch.as_tensor(np.ascontiguousarray(wl.Wtt[: lcut + 1]))
+    outb = {k: torch.empty((N, 2 * lcut + 1), dtype=torch.float64) for k in ("TT", "EB")}
+    binding.coupling_host(T, W, None, W, outb, band_lcut=lcut)
+    refb = oracle.coupling_band(wl.lmax, lcut, W.numpy(), None, W.numpy())
+    assert_parity(outb["TT"].numpy(), refb["TT"], "host band TT")
+    assert_parity(outb["EB"].numpy(), refb["EB"], "host band EB")
+    T.close()
+
+
+# ---------------------------------------------------------------- T3 full-size configs, sampled
+def _sample_pairs(lmax, n, seed, band=None):
+    rng = np.random.default_rng(seed)
+    l1 = rng.integers(0, lmax + 1, n)
+    if band is None:
+        l2 = rng.integers(0, lmax + 1, n)
+    else:
+        l2 = np.clip(l1 + rng.integers(-band, band + 1, n), 0, lmax)
+    # structured: corners, diagonal, l<2 edges, tile seams (multiples of 8/16/128), last rows/cols
+    edge = np.array([0, 1, 2, 3, 7, 8, 9, 127, 128, 129, lmax - 129, lmax - 128, lmax - 9, lmax - 8, lmax - 1, lmax])
+    edge = edge[(edge >= 0) & (edge <= lmax)]
+    e1, e2 = np.meshgrid(edge, edge, indexing="ij")
+    if band is not None:
+        keep = np.abs(e1 - e2) <= band
+        e1, e2 = e1[keep], e2[keep]
+    d = rng.integers(0, lmax + 1, 64)
+    l1 = np.concatenate([l1, e1.ravel(), d, d])
+    l2 = np.concatenate([l2, e2.ravel(), d, np.clip(d + 1, 0, lmax)])
+    return l1.astype(np.int32), l2.astype(np.int32)
+
+
+@pytest.mark.parametrize("cfg,npairs", [(1, 6000), (2, 3000), (3, 2500)])
+def test_full_size_configs_sampled(cfg, npairs):
+    """BASELINE.json configs 1-3 at full size, in the launch configuration bench.py times; outputs
+    sampled at random + structured pairs the oracle computes one by one."""
+    import torch
+    wl = windows.config(cfg)
+    T = binding.build_tables(wl.lmax)
+    out = binding.coupling_pol(T, _t(wl.Wtt), _t(wl.Wtp), _t(wl.Wpp))
+    torch.cuda.synchronize()
+    l1, l2 = _sample_pairs(wl.lmax, npairs, 100 + cfg)
+    ref = oracle.coupling_pairs(wl.l3max, wl.Wtt, wl.Wtp, wl.Wpp, l1, l2)
+    i1 = torch.as_tensor(l1.astype(np.int64)).cuda()
+    i2 = torch.as_tensor(l2.astype(np.int64)).cuda()
+    worst = {}
+    for k in BLOCKS:
+        got = out[k][i1, i2].cpu().numpy()
+        worst[k] = assert_parity(got, ref[k], "cfg%d %s" % (cfg, k))
+    # properties that hold at any size: Xi symmetry on a sampled set, BB == EE, l<2 zero
+    w1 = torch.as_tensor(2.0 * l1 + 1.0).cuda()
+    w2 = torch.as_tensor(2.0 * l2 + 1.0).cuda()
+    for k in BLOCKS:
+        a = out[k][i1, i2] * w1
+        b = out[k][i2, i1] * w2
+        assert torch.all((a - b).abs() <= 4e-16 * torch.maximum(a.abs(), b.abs())), k
+        if k != "TT":
+            assert torch.all(out[k][:2] == 0) and torch.all(out[k][:, :2] == 0)
+    assert torch.equal(out["BB"], out["EE"])
+    print("cfg%d worst (rel, abs-small):" % cfg, worst)
+    del out
+    T.close()
+
+
+def test_cfg4_band_full_size_sampled():
+    import torch
+    wl = windows.config(4)
+    lcut = wl.l3max
+    T = binding.build_tables(wl.lmax)
+    out = binding.coupling_band(T, lcut, _t(wl.Wtt), _t(wl.Wtp), _t(wl.Wpp))
+    torch.cuda.synchronize()
+    l1, l2 = _sample_pairs(wl.lmax, 3000, 104, band=lcut)
+    ref = oracle.coupling_pairs(lcut, wl.Wtt, wl.Wtp, wl.Wpp, l1, l2)
+    i1 = torch.as_tensor(l1.astype(np.int64)).cuda()
+    io = torch.as_tensor((l2.astype(np.int64) - l1 + lcut)).cuda()
+    for k in BLOCKS:
+        assert out[k].shape == (wl.lmax + 1, 2 * lcut + 1)
+        got = out[k][i1, io].cpu().numpy()
+        assert_parity(got, ref[k], "cfg4 %s" % k)
+    # rows 0 and lmax: out-of-range slots zero
+    assert torch.all(out["TT"][0, :lcut] == 0) and torch.all(out["TT"][-1, lcut + 1:] == 0)
+    T.close()
