@@ -1,0 +1,348 @@
+#!/usr/bin/env python
+"""bench.py -- the headline measurement (BASELINE.json `metric`).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 3]
+
+One "step" = one pass of the whole hot path (prepare -> fused l3 sweep -> mirrored writer) for
+TT+TE+EE+BB+EB on BASELINE.json configs[3] (lmax = 10000, l3 up to 20000, synthetic seeded windows),
+through the C ABI (tj_coupling_pol), inputs resident in HBM.  metric = evaluated l3 terms per second
+(upper triangle, even-J + odd-J terms).  Prints ONE JSON line (rank 0).
+
+N > 1 (torchrun): the path has no exchange step; every rank runs the same-size problem on its own
+window set (seed 3 + rank) -- weak scaling over independent window sets, no data-path collective.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "coupling-matrix l3-terms/sec (FP64) at lmax=10000, fraction of B200 FP64 peak"
+UNIT = "l3-terms/s"
+
+# FP64 roofline: 148 SMs x 64 FP64 lanes/clk (GB100: 4 SMSPs x 16 lanes) x SM clock.
+SM_COUNT = 148
+FP64_LANES_PER_SM = 64
+# algorithmic FP64 instructions per evaluated term
+INSTR_EVEN_POL, INSTR_ODD, INSTR_EVEN_TT = 8, 5, 2
+
+
+def _peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as fh:
+            return json.load(fh), "measured"
+    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi sampling DURING the timed region (B200_PROFILING.md clocks line)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index=0):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+        self.gpu = gpu_index
+
+    def start(self):
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(self.gpu), "--query-gpu=" + self.Q,
+                                       "--format=csv,noheader,nounits", "-lms", "100"],
+                                      stdout=self.f, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.p is None:
+            return out
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except Exception:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, mx, pw, reasons = [], [], [], set()
+        for line in self.f.read().splitlines():
+            c = [x.strip() for x in line.split(",")]
+            if len(c) < 9:
+                continue
+            try:
+                sm.append(float(c[1])); mx.append(float(c[2])); pw.append(float(c[3]))
+            except ValueError:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), c[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        try:
+            os.unlink(self.f.name)
+        except OSError:
+            pass
+        if sm:
+            # "under load" = samples in the upper half of the power range
+            thr = 0.5 * (max(pw) + min(pw)) if pw else 0
+            load = [s for s, w in zip(sm, pw) if w >= thr] or sm
+            out.update(sm_mhz=statistics.median(load), sm_max_mhz=max(mx), reasons=sorted(reasons),
+                       samples=len(sm), power_w_max=max(pw))
+        return out
+
+
+def _oracle_sample(lmax, cfg):
+    """Deterministic bounded sample of the workload for the CPU legs: every `stride`-th row, all columns."""
+    import numpy as np
+    stride = 251 if lmax >= 5000 else max(1, lmax // 40)
+    rows = np.arange(stride // 2, lmax + 1, stride, dtype=np.int32)
+    N = lmax + 1
+    l1 = np.repeat(rows, N)
+    l2 = np.tile(np.arange(N, dtype=np.int32), rows.size)
+    # terms the oracle evaluates: every l3 of the triangle range (both parities), per pair
+    lo = np.abs(l1.astype(np.int64) - l2)
+    hi = np.minimum(l1.astype(np.int64) + l2, 2 * lmax)
+    terms = int((hi - lo + 1).sum())
+    return l1, l2, terms, "cfg%d rows %d::%d (%d rows x %d cols, all blocks)" % (cfg, stride // 2, stride, rows.size, N)
+
+
+def time_oracle(wl, cfg, reps=1):
+    import oracle
+    l1, l2, terms, what = _oracle_sample(wl.lmax, cfg)
+    oracle.lib()
+    best = None
+    for _ in range(reps):
+        t0 = time.perf_counter()
+        oracle.coupling_pairs(wl.l3max, wl.Wtt, wl.Wtp, wl.Wpp, l1, l2)
+        dt = time.perf_counter() - t0
+        best = dt if best is None else min(best, dt)
+    return {"value": terms / best, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+            "sample": what, "sample_terms": terms, "sample_seconds": best}
+
+
+def run_reference(args):
+    """--impl reference: the oracle as it stands, on the host cores, on a bounded sample per step."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    from paper_2602_15605_b200 import windows
+    wl = windows.config(args.config)
+    import oracle
+    l1, l2, terms, what = _oracle_sample(wl.lmax, args.config)
+    oracle.lib()
+    for _ in range(min(args.warmup, 1)):
+        oracle.coupling_pairs(wl.l3max, wl.Wtt, wl.Wtp, wl.Wpp, l1[: l1.size // 8], l2[: l2.size // 8])
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle.coupling_pairs(wl.l3max, wl.Wtt, wl.Wtp, wl.Wpp, l1, l2)
+    dt = time.perf_counter() - t0
+    val = terms * args.steps / dt
+    line = {
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": wl.name, "lmax": wl.lmax, "l3max": wl.l3max, "blocks": "TT+TE+EE+BB+EB",
+                   "note": "each step = the oracle on a bounded row sample of the workload"},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle", "sample": what},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=3, help="BASELINE.json configs index (headline: 3)")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import numpy as np
+    import torch
+    from paper_2602_15605_b200 import binding, build, windows
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    dist = None
+    if world > 1:
+        import torch.distributed as dist_
+        dist = dist_
+        torch.cuda.set_device(local_rank)
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    else:
+        torch.cuda.set_device(0)
+    if rank == 0:
+        build.build()
+    if dist is not None:
+        dist.barrier()
+    binding.load_library()   # fails loudly if the CUDA library is missing: no fallback
+
+    base = windows.config(args.config)
+    if world > 1 and not base.band:
+        # each rank: its own window set of the same recipe (independent problems, weak scaling)
+        spec = {1: ((0.7, 30.0, 2.5), (0.5, 50.0, 3.0), False), 2: ((0.6, 40.0, 2.2), (0.45, 60.0, 2.8), True),
+                3: ((0.4, 80.0, 2.0), (0.35, 100.0, 2.4), False)}.get(args.config)
+        if spec is not None:
+            tt, tp, pp = windows.pol_windows(base.lmax, spec[0], spec[1], 0.05, args.config + rank, ripple=spec[2])
+            base = windows.Workload(base.name, base.lmax, base.l3max, False, True, tt, tp, pp)
+    wl = base
+    N = wl.lmax + 1
+    E, O, P = windows.term_counts(wl.lmax, wl.l3max)
+    terms = E + O
+    blocks = ("TT", "TE", "EE", "BB", "EB") if wl.pol else ("TT",)
+
+    T = binding.build_tables(wl.lmax, None if not wl.band else 2 * wl.lmax)
+    dW = [None if w is None else torch.as_tensor(w, dtype=torch.float64).cuda() for w in (wl.Wtt, wl.Wtp, wl.Wpp)]
+    width = (2 * wl.l3max + 1) if wl.band else N
+    out = {k: torch.empty((N, width), dtype=torch.float64, device="cuda") for k in blocks}
+    flush = torch.empty(512 * 1024 * 1024 // 8, dtype=torch.float64, device="cuda")
+
+    def step():
+        if wl.band:
+            binding.coupling_band(T, wl.l3max, *dW, want=blocks, out=out)
+        elif wl.pol:
+            binding.coupling_pol(T, *dW, want=blocks, out=out)
+        else:
+            binding.coupling_tt(T, dW[0], out["TT"])
+
+    def sync_all():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    binding.profile_enable(True)
+    for _ in range(max(args.warmup, 3)):
+        step()
+    sync_all()
+
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    time.sleep(0.3)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    kern = []
+    sync_all()
+    t_wall0 = time.perf_counter()
+    for i in range(args.steps):
+        flush.fill_(float(i))            # L2 flush between timed iterations (outside the event pair)
+        ev[i][0].record()
+        step()
+        ev[i][1].record()
+        kern.append(binding.profile_get())   # waits for this step's kernels (per-kernel device times)
+    sync_all()
+    t_wall = time.perf_counter() - t_wall0
+    clocks = sampler.stop()
+    step_ms = [a.elapsed_time(b) for a, b in ev]
+    total_ms = float(sum(step_ms))
+    if dist is not None:
+        t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    value = world * terms * args.steps / (total_ms * 1e-3)
+
+    # ---- roofline of the dominant kernel (the sweep), timed live with the library's CUDA events ----
+    sweep_ms = statistics.mean(k[1] for k in kern)
+    prep_ms = statistics.mean(k[0] for k in kern)
+    writer_ms = statistics.mean(k[2] for k in kern)
+    if wl.pol:
+        alg_instr = INSTR_EVEN_POL * E + INSTR_ODD * O
+        alg_flops = 12 * E + 6 * O
+    else:
+        alg_instr = INSTR_EVEN_TT * E
+        alg_flops = 3 * E
+    peaks, peak_kind = _peaks()
+    sm_max = float(clocks.get("sm_max_mhz") or peaks.get("sm_max_mhz", 1965.0))
+    peak_instr = SM_COUNT * FP64_LANES_PER_SM * sm_max * 1e6          # thread-instr/s at max boost
+    achieved = alg_instr / (sweep_ms * 1e-3)
+    probe = binding.fp64_probe(40000)
+    bytes_out = len(blocks) * N * width * 8
+    nmirror = len(blocks) - (1 if "BB" in blocks else 0)
+    writer_bytes = int(nmirror * 1.5 * N * width * 8 + (N * width * 8 if "BB" in blocks else 0))
+    roofline = {
+        "bound": "alu", "kernel": "sweep_kernel<R=8,TT|TE|EE|EB>" if wl.pol else "sweep_kernel<R=16,TT>",
+        "achieved": achieved / 1e12, "peak": peak_instr / 1e12, "unit": "T FP64 thread-instr/s",
+        "frac": achieved / peak_instr, "traffic": None,
+        "peak_source": "derived: %d SMs x %d FP64 lanes/clk x %.0f MHz (DESIGN.md 6; MEASURED_PEAKS.json has no FP64 entry)"
+                       % (SM_COUNT, FP64_LANES_PER_SM, sm_max),
+        "algorithmic_instr_per_launch": alg_instr, "algorithmic_flops_per_launch": alg_flops,
+        "achieved_tflops": alg_flops / (sweep_ms * 1e-3) / 1e12,
+        "measured_dfma_peak": probe / 1e12, "frac_of_measured_dfma": achieved / probe,
+        "kernel_ms": {"prepare": prep_ms, "sweep": sweep_ms, "writer": writer_ms},
+        "sweep_share_of_step": sweep_ms / (total_ms / args.steps) if world == 1 else None,
+        # writer: per mirrored block reads the upper triangle (N^2/2) and writes N^2; BB is one more N^2 write
+        "writer": {"bound": "hbm", "achieved": writer_bytes / (writer_ms * 1e-3) / 1e9, "peak": peaks.get("hbm_gbs"),
+                   "unit": "GB/s", "frac": writer_bytes / (writer_ms * 1e-3) / 1e9 / peaks.get("hbm_gbs"),
+                   "peak_kind": peak_kind, "algorithmic_bytes": writer_bytes},
+    }
+
+    # ---- end to end through the C ABI with HOST buffers (H2D + D2H inside the timed region) ----
+    e2e = None
+    if not args.no_e2e:
+        hW = [None if w is None else torch.as_tensor(w, dtype=torch.float64).pin_memory() for w in (wl.Wtt, wl.Wtp, wl.Wpp)]
+        hout = {k: torch.empty((N, width), dtype=torch.float64).pin_memory() for k in blocks}
+        del out
+        torch.cuda.empty_cache()
+        lc = wl.l3max if wl.band else None
+        binding.coupling_host(T, *hW, hout, band_lcut=lc)      # warm-up (pool growth, page faults)
+        sync_all()
+        n_e2e = max(1, min(args.steps, 3))
+        t0 = time.perf_counter()
+        for _ in range(n_e2e):
+            binding.coupling_host(T, *hW, hout, band_lcut=lc)  # synchronises internally
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        if dist is not None:
+            t = torch.tensor([dt], dtype=torch.float64, device="cuda")
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            dt = float(t.item())
+        e2e = {"value": world * terms * n_e2e / dt, "unit": UNIT,
+               "h2d_bytes_per_step": int(sum(w.numel() * 8 for w in hW if w is not None)),
+               "d2h_bytes_per_step": int(sum(v.numel() * 8 for v in hout.values())),
+               "ms_per_step": 1e3 * dt / n_e2e, "steps": n_e2e, "api": "tj_coupling_host (pinned host buffers)"}
+        del hout
+
+    cpu_baseline = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline and not wl.band:
+        cpu_baseline = time_oracle(wl, args.config)
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": total_ms / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": wl.name, "lmax": wl.lmax, "l3max": wl.l3max, "blocks": "+".join(blocks),
+                       "terms_even": E, "terms_odd": O, "pairs_upper": P,
+                       "pairs_per_s": world * P * args.steps / (total_ms * 1e-3),
+                       "l2": "512 MB flush written between timed steps; each step also writes %.1f GB of output" % (bytes_out / 1e9),
+                       "parallelism": "1 problem per GPU" if world > 1 else "single GPU"},
+            "roofline": roofline, "cpu_baseline": cpu_baseline, "e2e": e2e,
+            "gpu_launches": binding.launches_per_call(1) * args.steps,
+            "clocks": clocks, "wall_s_timed_region": t_wall, "step_ms": step_ms,
+            "context": {"paper_A100_TT_lmax1e4_s": 0.63, "paper_A100_EE_lmax1e4_s": 3.2,
+                        "note": "paper numbers (PAPER.md:242) are another machine's: context, not the target"},
+        }
+        print(json.dumps(line))
+    T.close()
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

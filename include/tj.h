@@ -124,6 +124,15 @@ int tj_sweep_counts(int l1, int l2, int l3max, int *te_lo, int *te_hi, int *to_l
  */
 int tj_fp64_probe(int iters, void *cuda_stream, double *h_thread_instr_per_s);
 
+/*
+ * Per-kernel timing for the roofline (bench.py): while enabled, every coupling call records CUDA events
+ * on its stream around its three kernels.  tj_profile_get waits for the most recent call made by the
+ * calling thread and returns the device time in milliseconds of  h_ms3[0] prepare (a2+a3),
+ * h_ms3[1] sweep (a4+a5), h_ms3[2] writer (a6).  TJ_EINVAL if no profiled call was made on this thread.
+ */
+int tj_profile_enable(int on);
+int tj_profile_get(double *h_ms3);
+
 /* Time of the last-enqueued work is the caller's to measure; this returns how many kernels the given
  * entry point launches per call (for bench.py's gpu_launches): which = 0 tt, 1 pol, 2 band. */
 int tj_launches_per_call(int which);

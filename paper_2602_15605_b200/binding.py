@@ -19,7 +19,8 @@ TJ_OK, TJ_EINVAL, TJ_ENOMEM, TJ_ECUDA = 0, -1, -2, -3
 SYMBOLS = (
     "tj_build_tables", "tj_free_tables", "tj_tables_info", "tj_tables_copy",
     "tj_coupling_tt", "tj_coupling_pol", "tj_coupling_band", "tj_coupling_host",
-    "tj_l3_range", "tj_sweep_counts", "tj_fp64_probe", "tj_launches_per_call", "tj_strerror",
+    "tj_l3_range", "tj_sweep_counts", "tj_fp64_probe", "tj_profile_enable", "tj_profile_get",
+    "tj_launches_per_call", "tj_strerror",
 )
 
 
@@ -55,6 +56,8 @@ def load_library() -> ctypes.CDLL:
     L.tj_l3_range.argtypes = [ci, ci, ci, ci, ip, ip, ip]
     L.tj_sweep_counts.argtypes = [ci, ci, ci, ip, ip, ip, ip]
     L.tj_fp64_probe.argtypes = [ci, vp, dp]
+    L.tj_profile_enable.argtypes = [ci]
+    L.tj_profile_get.argtypes = [dp]
     L.tj_launches_per_call.argtypes = [ci]
     L.tj_strerror.argtypes = [ci]
     L.tj_strerror.restype = ctypes.c_char_p
@@ -232,3 +235,14 @@ def fp64_probe(iters=20000, stream=None):
 
 def launches_per_call(which: int) -> int:
     return int(load_library().tj_launches_per_call(which))
+
+
+def profile_enable(on: bool) -> None:
+    _check(load_library().tj_profile_enable(1 if on else 0), "tj_profile_enable")
+
+
+def profile_get():
+    """(prepare_ms, sweep_ms, writer_ms) of this thread's most recent coupling call."""
+    arr = (ctypes.c_double * 3)()
+    _check(load_library().tj_profile_get(arr), "tj_profile_get")
+    return float(arr[0]), float(arr[1]), float(arr[2])

@@ -1,4 +1,5 @@
 // tj_api.cu -- the C ABI of libtj (include/tj.h): argument checks, stream-ordered scratch, launches.
+#include <atomic>
 #include <math.h>
 #include <mutex>
 #include <new>
@@ -36,6 +37,22 @@ void tune_pool_once()
         unsigned long long thr = ~0ull;
         cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &thr);
     });
+}
+
+// optional per-kernel timing of the most recent coupling call of this thread (tj_profile_*)
+std::atomic<int> g_profile{0};
+struct ProfEvents { cudaEvent_t ev[5]; bool have = false; bool valid = false; };
+thread_local ProfEvents g_prof;
+
+void prof_record(int i, cudaStream_t st)
+{
+    if (!g_profile.load(std::memory_order_relaxed)) return;
+    if (!g_prof.have) {
+        for (int k = 0; k < 5; ++k) cudaEventCreate(&g_prof.ev[k]);
+        g_prof.have = true;
+    }
+    cudaEventRecord(g_prof.ev[i], st);
+    if (i == 4) g_prof.valid = true;
 }
 
 int total_tiles(int lmax, int l3max, int R, bool banded)
@@ -282,6 +299,25 @@ int tj_fp64_probe(int iters, void *cuda_stream, double *h_thread_instr_per_s)
     return TJ_OK;
 }
 
+int tj_profile_enable(int on)
+{
+    g_profile.store(on ? 1 : 0);
+    return TJ_OK;
+}
+
+int tj_profile_get(double *h_ms3)
+{
+    if (!h_ms3) return TJ_EINVAL;
+    if (!g_prof.have || !g_prof.valid) return TJ_EINVAL;
+    TJ_CUDA(cudaEventSynchronize(g_prof.ev[4]), "tj_profile_get");
+    float a = 0.f, b = 0.f, c = 0.f;
+    TJ_CUDA(cudaEventElapsedTime(&a, g_prof.ev[0], g_prof.ev[1]), "tj_profile_get");
+    TJ_CUDA(cudaEventElapsedTime(&b, g_prof.ev[2], g_prof.ev[3]), "tj_profile_get");
+    TJ_CUDA(cudaEventElapsedTime(&c, g_prof.ev[3], g_prof.ev[4]), "tj_profile_get");
+    h_ms3[0] = a; h_ms3[1] = b; h_ms3[2] = c;
+    return TJ_OK;
+}
+
 int tj_launches_per_call(int which)
 {
     // prepare + sweep + writer; the band call adds no kernel (its zero-fill is a memset)
@@ -331,13 +367,16 @@ int run_coupling(const tj_tables *tables, int lcut, const double *d_Wtt, const d
     int *tile_start = (int *)(scratch + wbytes);
 
     int rc = TJ_OK;
+    prof_record(0, st);
     cudaError_t e = launch_prepare(T, d_Wtt, d_Wtp, d_Wpp, nW, wtt, wtp, wpp, tile_start, R, l3max_eff, banded, st);
+    prof_record(1, st);
     if (e == cudaSuccess && banded) {
         // slots of the band whose l2 falls outside 0..lmax (and everything the sweep does not own) are 0
         double *outs[5] = {d_TT, d_TE, d_EE, d_BB, d_EB};
         for (int k = 0; k < 5 && e == cudaSuccess; ++k)
             if (outs[k]) e = cudaMemsetAsync(outs[k], 0, sizeof(double) * per, st);
     }
+    prof_record(2, st);
     if (e == cudaSuccess) {
         SweepParams P;
         P.g = T.g; P.ginv = T.ginv; P.h = T.h; P.gA = T.gA; P.gB = T.gB; P.u3 = T.u3; P.isd = T.isd;
@@ -349,6 +388,7 @@ int run_coupling(const tj_tables *tables, int lcut, const double *d_Wtt, const d
         P.lmax = T.lmax; P.l3max = l3max_eff; P.nbands = nb; P.lcut = banded ? lcut : -1; P.ld = ld;
         e = launch_sweep(P, mask, ntiles, st);
     }
+    prof_record(3, st);
     if (e == cudaSuccess) {
         WriterParams W;
         memset(&W, 0, sizeof(W));
@@ -364,6 +404,7 @@ int run_coupling(const tj_tables *tables, int lcut, const double *d_Wtt, const d
         W.tile_band = banded ? ((lcut + 31) / 32 + 1 < W.ntile - 1 ? (lcut + 31) / 32 + 1 : W.ntile - 1) : W.ntile - 1;
         e = launch_writer(W, st);
     }
+    prof_record(4, st);
     if (e != cudaSuccess) rc = cuda_fail(e, "coupling");
     cudaFreeAsync(scratch, st);
     return rc;

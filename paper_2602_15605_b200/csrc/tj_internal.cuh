@@ -20,7 +20,10 @@ constexpr int GUARD_HI = 768;
 // A thread owns R pairs on ONE anti-diagonal: (l1, l2) = (a+i, c-i), i = 0..R-1, a = band*R.
 // Lanes run along c, so a warp covers rows a..a+R-1 and a skewed window of 32+R-1 columns.
 constexpr int SWEEP_THREADS = 128;   // columns c per CTA
-constexpr int R_POL = 8;             // pairs per thread, fused TT+TE+EE(+EB) sweep
+#ifndef TJ_R_POL
+#define TJ_R_POL 8
+#endif
+constexpr int R_POL = TJ_R_POL;      // pairs per thread, fused TT+TE+EE(+EB) sweep
 constexpr int R_TT = 16;             // pairs per thread, TT-only sweep
 
 // mask bits of the blocks one sweep computes

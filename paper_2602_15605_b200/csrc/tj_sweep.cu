@@ -26,8 +26,22 @@ namespace {
 
 __device__ __forceinline__ double ldg(const double *p) { return __ldg(p); }
 
+// L1 prefetch of a table line the sweep will reach TJ_PF unrolled blocks from now (0 = off)
+#ifndef TJ_PF
+#define TJ_PF 0
+#endif
+#ifndef TJ_MINB
+#define TJ_MINB 3
+#endif
+__device__ __forceinline__ void pf(const double *p)
+{
+#if TJ_PF > 0
+    asm volatile("prefetch.global.L1 [%0];" ::"l"(p));
+#endif
+}
+
 template <int R, int MASK>
-__global__ void __launch_bounds__(SWEEP_THREADS) sweep_kernel(const __grid_constant__ SweepParams P)
+__global__ void __launch_bounds__(SWEEP_THREADS, TJ_MINB) sweep_kernel(const __grid_constant__ SweepParams P)
 {
     constexpr bool kTT = (MASK & M_TT) != 0, kTE = (MASK & M_TE) != 0, kEE = (MASK & M_EE) != 0,
                    kEB = (MASK & M_EB) != 0;
@@ -86,22 +100,31 @@ __global__ void __launch_bounds__(SWEEP_THREADS) sweep_kernel(const __grid_const
             for (int k = 1; k < R; ++k) wa[k] = ldg(pa + k);                       // G[k] = gA[a-t0+k]
 #pragma unroll
             for (int i = 0; i < R - 1; ++i) wb[(R - i) % R] = ldg(pb + (R - 1 - i));  // H[-i] = gA[c-t0-i]
+            // software pipeline: the raw table values of substep u+1 are loaded while substep u computes
+            double xa = ldg(pa), xb = ldg(pb), xh = ldg(ph), xg = ldg(pg), xw = ldg(pw), xu = ldg(pu);
             for (int blk = 0; blk < nblk; ++blk) {
 #pragma unroll
                 for (int u = 0; u < R; ++u) {
-                    wa[(R - u) % R] = ldg(pa - u);
-                    wb[(R + 1 - u) % R] = ldg(pb - u);
-                    const double hg = __dmul_rn(ldg(ph - u), ldg(pg + u));
-                    const double q3 = __dmul_rn(ldg(pw - 2 * u), hg);
-                    const double c3 = ldg(pu - 2 * u);
+                    wa[(R - u) % R] = xa;
+                    wb[(R + 1 - u) % R] = xb;
+                    const double hg = __dmul_rn(xh, xg);
+                    const double q3 = __dmul_rn(xw, hg);
+                    const double c3 = xu;
+                    xa = ldg(pa - (u + 1)); xb = ldg(pb - (u + 1)); xh = ldg(ph - (u + 1)); xg = ldg(pg + (u + 1));
+                    xw = ldg(pw - 2 * (u + 1)); xu = ldg(pu - 2 * (u + 1));
+                    // op-major order: consecutive FP64 instructions share c3 / q3 in one operand slot, so
+                    // the register-file reuse cache serves it and no instruction needs 3 bank reads
+                    double r[R], e[R];
 #pragma unroll
-                    for (int i = 0; i < R; ++i) {
-                        const double r = __dmul_rn(wa[(i - u + R) % R], wb[(2 * R - i - u) % R]);
-                        const double e = __dsub_rn(c3, c12[i]);
-                        const double re = __dmul_rn(r, e);
-                        const double ree = __dmul_rn(re, e);
-                        acc[i] = __fma_rn(ree, q3, acc[i]);
-                    }
+                    for (int i = 0; i < R; ++i) r[i] = __dmul_rn(wa[(i - u + R) % R], wb[(2 * R - i - u) % R]);
+#pragma unroll
+                    for (int i = 0; i < R; ++i) e[i] = __dsub_rn(c3, c12[i]);
+#pragma unroll
+                    for (int i = 0; i < R; ++i) r[i] = __dmul_rn(r[i], e[i]);
+#pragma unroll
+                    for (int i = 0; i < R; ++i) r[i] = __dmul_rn(r[i], e[i]);
+#pragma unroll
+                    for (int i = 0; i < R; ++i) acc[i] = __fma_rn(r[i], q3, acc[i]);
                 }
                 pa -= R; pb -= R; ph -= R; pg += R; pw -= 2 * R; pu -= 2 * R;
             }
@@ -149,30 +172,51 @@ __global__ void __launch_bounds__(SWEEP_THREADS) sweep_kernel(const __grid_const
             for (int k = 1; k < R; ++k) wa[k] = ldg(pa + k);
 #pragma unroll
             for (int i = 0; i < R - 1; ++i) wb[(R - i) % R] = ldg(pb + (R - 1 - i));
+            double xa = ldg(pa), xb = ldg(pb), xh = ldg(ph), xg = ldg(pg);
+            double xtt = kTT ? ldg(pwtt) : 0.0, xtp = kTE ? ldg(pwtp) : 0.0, xpp = kEE ? ldg(pwpp) : 0.0;
+            double xu = kA2 ? ldg(pu) : 0.0;
             for (int blk = 0; blk < nblk; ++blk) {
 #pragma unroll
                 for (int u = 0; u < R; ++u) {
-                    wa[(R - u) % R] = ldg(pa - u);
-                    wb[(R + 1 - u) % R] = ldg(pb - u);
-                    const double hg = __dmul_rn(ldg(ph - u), ldg(pg + u));
-                    double q0 = 0.0, q1 = 0.0, q2 = 0.0, c3 = 0.0;
-                    if (kTT) q0 = __dmul_rn(ldg(pwtt - 2 * u), hg);
-                    if (kTE) q1 = __dmul_rn(ldg(pwtp - 2 * u), hg);
-                    if (kEE) q2 = __dmul_rn(ldg(pwpp - 2 * u), hg);
-                    if (kA2) c3 = ldg(pu - 2 * u);
+                    wa[(R - u) % R] = xa;
+                    wb[(R + 1 - u) % R] = xb;
+                    const double hg = __dmul_rn(xh, xg);
+                    double q0 = 0.0, q1 = 0.0, q2 = 0.0;
+                    if (kTT) q0 = __dmul_rn(xtt, hg);
+                    if (kTE) q1 = __dmul_rn(xtp, hg);
+                    if (kEE) q2 = __dmul_rn(xpp, hg);
+                    const double c3 = xu;
+                    xa = ldg(pa - (u + 1)); xb = ldg(pb - (u + 1)); xh = ldg(ph - (u + 1)); xg = ldg(pg + (u + 1));
+                    if (kTT) xtt = ldg(pwtt - 2 * (u + 1));
+                    if (kTE) xtp = ldg(pwtp - 2 * (u + 1));
+                    if (kEE) xpp = ldg(pwpp - 2 * (u + 1));
+                    if (kA2) xu = ldg(pu - 2 * (u + 1));
+                    // op-major order (see the odd branch): q0/q1/q2/c3 stay in the operand reuse cache
+                    double r[R], A2[kA2 ? R : 1];
 #pragma unroll
-                    for (int i = 0; i < R; ++i) {
-                        const double r = __dmul_rn(wa[(i - u + R) % R], wb[(2 * R - i - u) % R]);
-                        if (kTT) att[i] = __fma_rn(r, q0, att[i]);
-                        if (kA2) {
-                            const double d1 = __dsub_rn(c3, c12[i]);
-                            const double A2 = __fma_rn(d1, d1, -kk[i]);
-                            const double rA = __dmul_rn(r, A2);
-                            if (kTE) ate[i] = __fma_rn(rA, q1, ate[i]);
-                            if (kEE) {
-                                const double rAA = __dmul_rn(rA, A2);
-                                aee[i] = __fma_rn(rAA, q2, aee[i]);
-                            }
+                    for (int i = 0; i < R; ++i) r[i] = __dmul_rn(wa[(i - u + R) % R], wb[(2 * R - i - u) % R]);
+                    if (kA2) {
+#pragma unroll
+                        for (int i = 0; i < R; ++i) A2[i] = __dsub_rn(c3, c12[i]);
+                    }
+                    if (kTT) {
+#pragma unroll
+                        for (int i = 0; i < R; ++i) att[i] = __fma_rn(r[i], q0, att[i]);
+                    }
+                    if (kA2) {
+#pragma unroll
+                        for (int i = 0; i < R; ++i) A2[i] = __fma_rn(A2[i], A2[i], -kk[i]);
+#pragma unroll
+                        for (int i = 0; i < R; ++i) r[i] = __dmul_rn(r[i], A2[i]);
+                        if (kTE) {
+#pragma unroll
+                            for (int i = 0; i < R; ++i) ate[i] = __fma_rn(r[i], q1, ate[i]);
+                        }
+                        if (kEE) {
+#pragma unroll
+                            for (int i = 0; i < R; ++i) r[i] = __dmul_rn(r[i], A2[i]);
+#pragma unroll
+                            for (int i = 0; i < R; ++i) aee[i] = __fma_rn(r[i], q2, aee[i]);
                         }
                     }
                 }
