@@ -174,7 +174,7 @@ def main():
 
     import numpy as np
     import torch
-    from paper_2602_15605_b200 import binding, build, windows
+    from paper_2602_15605_b200 import binding, build, shard, windows
 
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
@@ -199,7 +199,8 @@ def main():
         spec = {1: ((0.7, 30.0, 2.5), (0.5, 50.0, 3.0), False), 2: ((0.6, 40.0, 2.2), (0.45, 60.0, 2.8), True),
                 3: ((0.4, 80.0, 2.0), (0.35, 100.0, 2.4), False)}.get(args.config)
         if spec is not None:
-            tt, tp, pp = windows.pol_windows(base.lmax, spec[0], spec[1], 0.05, args.config + rank, ripple=spec[2])
+            seed = shard.window_seed(args.config, shard.assign_window_sets(world, world, rank)[0])
+            tt, tp, pp = windows.pol_windows(base.lmax, spec[0], spec[1], 0.05, seed, ripple=spec[2])
             base = windows.Workload(base.name, base.lmax, base.l3max, False, True, tt, tp, pp)
     wl = base
     N = wl.lmax + 1
@@ -250,11 +251,8 @@ def main():
     clocks = sampler.stop()
     step_ms = [a.elapsed_time(b) for a, b in ev]
     total_ms = float(sum(step_ms))
-    if dist is not None:
-        t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
-    value = world * terms * args.steps / (total_ms * 1e-3)
+    total_ms = shard.max_over_ranks(total_ms, dist, "cuda")
+    value = shard.whole_job_throughput(terms, args.steps, total_ms, world)
 
     # ---- roofline of the dominant kernel (the sweep), timed live with the library's CUDA events ----
     sweep_ms = statistics.mean(k[1] for k in kern)
@@ -277,7 +275,10 @@ def main():
     roofline = {
         "bound": "alu", "kernel": "sweep_kernel<R=8,TT|TE|EE|EB>" if wl.pol else "sweep_kernel<R=16,TT>",
         "achieved": achieved / 1e12, "peak": peak_instr / 1e12, "unit": "T FP64 thread-instr/s",
-        "frac": achieved / peak_instr, "traffic": None,
+        "frac": achieved / peak_instr,
+        # dram__bytes_read.sum + dram__bytes_write.sum of one sweep launch, from the ncu --set full capture
+        # profiles/r1_ncu_full_cfg3.md (config 3 only; other configs: not captured)
+        "traffic": 1.572e9 if (args.config == 3 and wl.pol) else None,
         "peak_source": "derived: %d SMs x %d FP64 lanes/clk x %.0f MHz (DESIGN.md 6; MEASURED_PEAKS.json has no FP64 entry)"
                        % (SM_COUNT, FP64_LANES_PER_SM, sm_max),
         "algorithmic_instr_per_launch": alg_instr, "algorithmic_flops_per_launch": alg_flops,
@@ -307,10 +308,7 @@ def main():
             binding.coupling_host(T, *hW, hout, band_lcut=lc)  # synchronises internally
         torch.cuda.synchronize()
         dt = time.perf_counter() - t0
-        if dist is not None:
-            t = torch.tensor([dt], dtype=torch.float64, device="cuda")
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            dt = float(t.item())
+        dt = shard.max_over_ranks(dt, dist, "cuda")
         e2e = {"value": world * terms * n_e2e / dt, "unit": UNIT,
                "h2d_bytes_per_step": int(sum(w.numel() * 8 for w in hW if w is not None)),
                "d2h_bytes_per_step": int(sum(v.numel() * 8 for v in hout.values())),

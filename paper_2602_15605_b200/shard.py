@@ -1,0 +1,35 @@
+"""Multi-GPU plumbing: the path has no exchange step (every (l1,l2) entry and every window set is
+independent), so N GPUs run N independent problems -- one process per GPU, window
+sets dealt round-robin, no data-path collective.  The only communication is the timing reduction
+(max over ranks) and a barrier, done with torch.distributed (NCCL on GPUs, gloo in the CPU tests).
+
+Nothing here touches the arithmetic of the method.
+"""
+from __future__ import annotations
+
+
+def assign_window_sets(n_sets: int, world: int, rank: int) -> list[int]:
+    """Indices of the window sets rank `rank` of `world` computes (round-robin deal)."""
+    if world <= 0 or not (0 <= rank < world) or n_sets < 0:
+        raise ValueError("bad (n_sets, world, rank) = (%r, %r, %r)" % (n_sets, world, rank))
+    return list(range(rank, n_sets, world))
+
+
+def window_seed(config_seed: int, set_index: int) -> int:
+    """Seed of window set `set_index` of a config (set 0 is the BASELINE.json seed itself)."""
+    return int(config_seed) + int(set_index)
+
+
+def max_over_ranks(value: float, dist=None, device=None) -> float:
+    """MAX all-reduce of a scalar (the device-timed duration) -- identity when not distributed."""
+    if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
+        return float(value)
+    import torch
+    t = torch.tensor([float(value)], dtype=torch.float64, device=device or "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_throughput(units_per_rank: float, steps: int, ms_max: float, world: int) -> float:
+    """units all ranks processed / the slowest rank's time (weak scaling, same work per rank)."""
+    return world * units_per_rank * steps / (ms_max * 1e-3)

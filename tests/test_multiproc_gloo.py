@@ -1,0 +1,73 @@
+"""World-size-2 CPU test (gloo) of the N > 1 host logic: window-set sharding covers every set exactly
+once with no overlap, the timing reduction is a max over ranks, and the whole-job throughput formula
+uses it.  No GPU, no kernels: the data path has no collective to test."""
+import os
+import socket
+import sys
+
+import pytest
+import torch
+import torch.distributed as dist
+import torch.multiprocessing as mp
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _free_port():
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    p = s.getsockname()[1]
+    s.close()
+    return p
+
+
+def _worker(rank, world, port, n_sets, q):
+    sys.path.insert(0, ROOT)
+    from paper_2602_15605_b200 import shard, windows
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    mine = shard.assign_window_sets(n_sets, world, rank)
+    # every rank draws its own window set of the config-1 recipe
+    seeds = [shard.window_seed(1, k) for k in mine]
+    sums = [float(windows.pol_windows(20, (0.7, 30.0, 2.5), (0.5, 50.0, 3.0), 0.05, sd)[0].sum()) for sd in seeds]
+    gathered = [None] * world
+    dist.all_gather_object(gathered, (mine, sums))
+    fake_ms = 10.0 + 5.0 * rank
+    mx = shard.max_over_ranks(fake_ms, dist)
+    dist.barrier()
+    q.put((rank, gathered, mx, shard.whole_job_throughput(1000.0, 4, mx, world)))
+    dist.destroy_process_group()
+
+
+def test_window_set_sharding_and_timing_reduction_world2():
+    world, n_sets = 2, 5
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_worker, args=(r, world, port, n_sets, q)) for r in range(world)]
+    for p in procs:
+        p.start()
+    res = [q.get(timeout=120) for _ in range(world)]
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    for rank, gathered, mx, thr in res:
+        allsets = sorted(k for mine, _ in gathered for k in mine)
+        assert allsets == list(range(n_sets))                      # exact cover, no overlap
+        assert mx == 15.0                                          # max over ranks
+        assert thr == pytest.approx(2 * 1000.0 * 4 / 15e-3)
+        # different sets -> different windows (distinct seeds)
+        flat = [s for _, sums in gathered for s in sums]
+        assert len(set(flat)) == n_sets
+
+
+def test_assign_window_sets_edge_cases():
+    from paper_2602_15605_b200 import shard
+    assert shard.assign_window_sets(0, 4, 1) == []
+    assert shard.assign_window_sets(3, 8, 5) == []
+    assert shard.assign_window_sets(3, 8, 2) == [2]
+    assert sorted(sum((shard.assign_window_sets(17, 4, r) for r in range(4)), [])) == list(range(17))
+    with pytest.raises(ValueError):
+        shard.assign_window_sets(3, 2, 2)
+    assert shard.max_over_ranks(3.5, None) == 3.5
