@@ -4,6 +4,7 @@
 #include <mutex>
 #include <new>
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include "tj_internal.cuh"
@@ -55,6 +56,17 @@ void prof_record(int i, cudaStream_t st)
     if (i == 4) g_prof.valid = true;
 }
 
+// which sweep kernel serves the calls: 0 = bulk-copy staged (default), 1 = L1-path kernel of tj_sweep.cu.
+// TJ_SWEEP_IMPL=l1 in the environment selects the latter (A/B measurements only).
+int sweep_impl()
+{
+    static const int impl = [] {
+        const char *v = getenv("TJ_SWEEP_IMPL");
+        return (v && strcmp(v, "l1") == 0) ? 1 : 0;
+    }();
+    return impl;
+}
+
 int total_tiles(int lmax, int l3max, int R, bool banded)
 {
     long long n = 0;
@@ -99,7 +111,7 @@ int tj_build_tables(int lmax, int l3max, void *cuda_stream, tj_tables **out)
     T.l3max = l3max;
     T.pmax = 2 * lmax + 1;
     T.np_alloc = GUARD_LO + T.pmax + 1 + GUARD_HI;
-    T.nl_alloc = GUARD_LO + 2 * lmax + 1 + GUARD_HI;
+    T.nl_alloc = GUARD_LO + 2 * lmax + 2 + GUARD_HI;   // even, like np_alloc: every table's index 0 is 16-byte aligned (bulk copies)
     size_t n = (size_t)5 * T.np_alloc + (size_t)2 * T.nl_alloc;
     cudaError_t e = cudaMalloc((void **)&T.base, n * sizeof(double));
     if (e != cudaSuccess) { delete h; return cuda_fail(e, "tj_build_tables/cudaMalloc"); }
@@ -386,7 +398,7 @@ int run_coupling(const tj_tables *tables, int lcut, const double *d_Wtt, const d
         P.TT = d_TT; P.TE = d_TE; P.EE = ee; P.EB = d_EB;
         P.tile_start = tile_start;
         P.lmax = T.lmax; P.l3max = l3max_eff; P.nbands = nb; P.lcut = banded ? lcut : -1; P.ld = ld;
-        e = launch_sweep(P, mask, ntiles, st);
+        e = sweep_impl() == 0 ? launch_sweep_tma(P, mask, ntiles, st) : launch_sweep(P, mask, ntiles, st);
     }
     prof_record(3, st);
     if (e == cudaSuccess) {

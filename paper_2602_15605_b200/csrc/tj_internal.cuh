@@ -85,7 +85,8 @@ cudaError_t launch_build_tables(const Tables &T, cudaStream_t st);
 cudaError_t launch_prepare(const Tables &T, const double *d_Wtt, const double *d_Wtp, const double *d_Wpp, int nW,
                            double *wtt, double *wtp, double *wpp, int *tile_start, int R, int l3max_eff, bool banded,
                            cudaStream_t st);
-cudaError_t launch_sweep(const SweepParams &P, int mask, int total_tiles, cudaStream_t st);
+cudaError_t launch_sweep(const SweepParams &P, int mask, int total_tiles, cudaStream_t st);      // tables via L1 (tj_sweep.cu)
+cudaError_t launch_sweep_tma(const SweepParams &P, int mask, int total_tiles, cudaStream_t st);  // tables via bulk copies to smem
 cudaError_t launch_writer(const WriterParams &P, cudaStream_t st);
 cudaError_t launch_fp64_probe(int iters, double *d_sink, int blocks, int threads, cudaStream_t st);
 
