@@ -56,17 +56,6 @@ void prof_record(int i, cudaStream_t st)
     if (i == 4) g_prof.valid = true;
 }
 
-// which sweep kernel serves the calls: 0 = bulk-copy staged (default), 1 = L1-path kernel of tj_sweep.cu.
-// TJ_SWEEP_IMPL=l1 in the environment selects the latter (A/B measurements only).
-int sweep_impl()
-{
-    static const int impl = [] {
-        const char *v = getenv("TJ_SWEEP_IMPL");
-        return (v && strcmp(v, "l1") == 0) ? 1 : 0;
-    }();
-    return impl;
-}
-
 int total_tiles(int lmax, int l3max, int R, bool banded)
 {
     long long n = 0;
@@ -357,7 +346,7 @@ int run_coupling(const tj_tables *tables, int lcut, const double *d_Wtt, const d
     if (!d_TE && !ee && !d_EB) mask = M_TT;
     else if (d_TT) mask = M_TT | M_TE | M_EE | M_EB;
     else mask = M_TE | M_EE | M_EB;
-    const int R = (mask == M_TT) ? R_TT : R_POL;
+    const int R = sweep_R(mask, banded);
     const int l3max_eff = banded ? lcut : T.l3max;
     const long long N = (long long)T.lmax + 1;
     const long long ld = banded ? (long long)(2 * lcut + 1) : N;
@@ -398,7 +387,7 @@ int run_coupling(const tj_tables *tables, int lcut, const double *d_Wtt, const d
         P.TT = d_TT; P.TE = d_TE; P.EE = ee; P.EB = d_EB;
         P.tile_start = tile_start;
         P.lmax = T.lmax; P.l3max = l3max_eff; P.nbands = nb; P.lcut = banded ? lcut : -1; P.ld = ld;
-        e = sweep_impl() == 0 ? launch_sweep_tma(P, mask, ntiles, st) : launch_sweep(P, mask, ntiles, st);
+        e = launch_sweep(P, mask, ntiles, st);
     }
     prof_record(3, st);
     if (e == cudaSuccess) {

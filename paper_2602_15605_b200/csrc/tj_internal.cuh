@@ -20,10 +20,8 @@ constexpr int GUARD_HI = 768;
 // A thread owns R pairs on ONE anti-diagonal: (l1, l2) = (a+i, c-i), i = 0..R-1, a = band*R.
 // Lanes run along c, so a warp covers rows a..a+R-1 and a skewed window of 32+R-1 columns.
 constexpr int SWEEP_THREADS = 128;   // columns c per CTA
-#ifndef TJ_R_POL
-#define TJ_R_POL 8
-#endif
-constexpr int R_POL = TJ_R_POL;      // pairs per thread, fused TT+TE+EE(+EB) sweep
+constexpr int R_POL = 12;           // pairs per thread, fused TT+TE+EE(+EB) sweep, dense storage
+constexpr int R_POL_BAND = 8;       // same, band-limited (short sweeps)
 constexpr int R_TT = 16;             // pairs per thread, TT-only sweep
 
 // mask bits of the blocks one sweep computes
@@ -85,8 +83,8 @@ cudaError_t launch_build_tables(const Tables &T, cudaStream_t st);
 cudaError_t launch_prepare(const Tables &T, const double *d_Wtt, const double *d_Wtp, const double *d_Wpp, int nW,
                            double *wtt, double *wtp, double *wpp, int *tile_start, int R, int l3max_eff, bool banded,
                            cudaStream_t st);
-cudaError_t launch_sweep(const SweepParams &P, int mask, int total_tiles, cudaStream_t st);      // tables via L1 (tj_sweep.cu)
-cudaError_t launch_sweep_tma(const SweepParams &P, int mask, int total_tiles, cudaStream_t st);  // tables via bulk copies to smem
+int sweep_R(int mask, bool banded);   // pairs per thread (= rows per band) of the sweep that serves `mask`
+cudaError_t launch_sweep(const SweepParams &P, int mask, int total_tiles, cudaStream_t st);
 cudaError_t launch_writer(const WriterParams &P, cudaStream_t st);
 cudaError_t launch_fp64_probe(int iters, double *d_sink, int blocks, int threads, cudaStream_t st);
 

@@ -10,47 +10,120 @@
 //   odd step t (l3 = s-2t-1, t = 0..min(l1,l2)-1):
 //       Z^2 = ginv[s-t] gB[t] gA[l1-t] gA[l2-t],  e = u_l3 - u_l1 - u_l2 + 2
 //       S_EB += W'_PP[l3] Z^2 e^2
-//   Xi_TT = S_TT,  Xi_TE = S_TE/(2 sqrt(D)),  Xi_EE = S_EE/(4D),  Xi_EB = S_EB/(4D),  D = D_l1 D_l2.
+//   Xi_TT = S_TT,  Xi_TE = S_TE/(2 sqrt D),  Xi_EE = S_EE/(4D),  Xi_EB = S_EB/(4D),  D = D_l1 D_l2.
 //
 // Mapping to the machine.  A thread owns R pairs on ONE anti-diagonal,
 // (l1,l2) = (a+i, c-i), so s, l3, h[s-t] g[t], the three W'[l3] and u_l3 are per-THREAD values per step,
-// and the two per-pair table factors g[a+i-t], g[c-i-t] slide through two R-deep register rings:
-// each step loads ONE new element per ring.  Lanes run along c: the per-row loads are warp broadcasts,
-// everything else is consecutive doubles (no bank or sector conflicts).  Per even step a thread issues
-// 8R+4 FP64 instructions against 8 loads.  Steps outside a pair's triangle (or beyond l3max) hit the zero
-// guard bands of the tables / windows and add exact zeros, so the warp runs one branch-free t range.
+// and the two per-pair table factors g[a+i-t], g[c-i-t] slide through two R-deep register rings: each
+// step reads ONE new element per ring.  Lanes run along c.  Steps outside a pair's triangle (or beyond
+// l3max) hit the zero guard bands of the tables / windows and add exact zeros, so a warp runs one
+// branch-free t range.
+//
+// Where the per-step table values come from: shared memory, filled by the bulk-copy engine
+// (cp.async.bulk + mbarrier), one private double-buffered pipeline PER WARP.  A warp walks its t range in
+// STAGES of TS steps.  For one stage every value the warp will read is a contiguous slice of a table:
+//
+//     row ring      g [a - t]           TS          doubles   (broadcast)
+//     step factor   g [t]               TS          doubles   (broadcast)
+//     column ring   g [cw-R+1+j - t]    TS+31       doubles   (lane j)
+//     1/(J+1)g(p)   h [a+cw+j - t]      TS+31       doubles
+//     windows, u3   W'[a+cw+j - 2t]     2(TS-1)+32  doubles each
+//
+// (odd-J branch: gA, gB, gA, ginv, W'_PP and u3 at l3 = s-2t-1).  Lane 0 asks the copy engine for the
+// slices of stage k+2 as soon as the warp has finished stage k; the copies land while the warp computes
+// stage k+1, and completion is signalled through the buffer's mbarrier (transaction bytes).  The inner
+// loop then reads shared memory only: no L1 miss can stall it, an address is one 32-bit register plus an
+// immediate, and warps stay independent of each other (no CTA barrier; a warp whose columns lie beyond
+// lmax leaves at once, and every warp keeps its own first step for band-limited windows).
+//
+// Issue-slot budget (measured): an FP64 instruction takes 2 issue cycles of its SM
+// sub-partition, 3 if it reads three distinct registers none of which the operand reuse cache serves, and
+// every other instruction (LDS, integer) costs about 1.45 cycles of FP64 time.  Hence: as many pairs per
+// thread as registers allow (R = 12 at 2 CTAs/SM for dense sweeps), and, with PIPE, the TE/EE
+// accumulations of step t are issued at the start of step t+1, when all their inputs are ready, so that
+// the R FMAs of one window are adjacent and share q through the reuse cache.
+//
+// Bulk copies need 16-byte aligned source, destination and size; table slices start at any double, so a slice
+// whose first index is odd is fetched from the even index below it and the consumers add that parity `e` to
+// their offsets.  Stages advance by TS (even), so `e` is fixed per array for the whole walk.
 #include "tj_internal.cuh"
 
 namespace tj {
 namespace {
 
-__device__ __forceinline__ double ldg(const double *p) { return __ldg(p); }
+constexpr int NBUF = 2;   // buffers per warp
+constexpr int PAD = 2;    // doubles in front of each slice: the software-pipelined read of "step TS" lands here
 
-// L1 prefetch of a table line the sweep will reach TJ_PF unrolled blocks from now (0 = off)
-#ifndef TJ_PF
-#define TJ_PF 0
-#endif
-#ifndef TJ_MINB
-#define TJ_MINB 3
-#endif
-__device__ __forceinline__ void pf(const double *p)
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint32_t bar, int count)
 {
-#if TJ_PF > 0
-    asm volatile("prefetch.global.L1 [%0];" ::"l"(p));
-#endif
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
+{
+    uint32_t done;
+    do {
+        asm volatile(
+            "{\n\t.reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(done)
+            : "r"(bar), "r"(parity)
+            : "memory");
+    } while (!done);
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t bytes, uint32_t bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+                 "l"(src), "r"(bytes), "r"(bar)
+                 : "memory");
 }
 
-template <int R, int MASK>
-__global__ void __launch_bounds__(SWEEP_THREADS, TJ_MINB) sweep_kernel(const __grid_constant__ SweepParams P)
+// capacities (doubles, all even) of the slices inside one stage buffer
+template <int TS> struct Lay {
+    static constexpr int CA = PAD + TS + 2;            // row ring / step factor
+    static constexpr int CB = PAD + TS + 32 + 2;       // column ring / h
+    static constexpr int CW = PAD + 2 * TS + 32 + 2;   // windows, u3
+    static constexpr int OA = 0, OG = OA + CA, OB = OG + CA, OH = OB + CB;
+    static constexpr int OW0 = OH + CB, OW1 = OW0 + CW, OW2 = OW1 + CW, OU = OW2 + CW;
+    static constexpr int BUFD = OU + CW;               // doubles per buffer
+};
+
+// one slice: n doubles starting at table index i0 (any parity) -> buffer offset off (+PAD)
+__device__ __forceinline__ uint32_t slice(uint32_t buf, int off, const double *tab, int i0, int n, uint32_t bar)
+{
+    const int ie = i0 & ~1;                 // even index at or below i0 (two's complement: also for i0 < 0)
+    const int cnt = (n + (i0 - ie) + 1) & ~1;
+    bulk_g2s(buf + (uint32_t)(off + PAD) * 8u, tab + ie, (uint32_t)cnt * 8u, bar);
+    return (uint32_t)cnt * 8u;
+}
+__device__ __forceinline__ int slice_bytes(int i0, int n)
+{
+    const int ie = i0 & ~1;
+    return ((n + (i0 - ie) + 1) & ~1) * 8;
+}
+
+template <int R, int MASK, int TS, int MINB, bool PIPE>
+__global__ void __launch_bounds__(SWEEP_THREADS, MINB) sweep_tma_kernel(const __grid_constant__ SweepParams P)
 {
     constexpr bool kTT = (MASK & M_TT) != 0, kTE = (MASK & M_TE) != 0, kEE = (MASK & M_EE) != 0,
                    kEB = (MASK & M_EB) != 0;
     constexpr bool kEven = kTT || kTE || kEE;
     constexpr bool kA2 = kTE || kEE;
+    using L = Lay<TS>;
+    static_assert(TS % R == 0 && TS % 2 == 0, "stage length: a multiple of R and even");
+
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    constexpr int NWARP = SWEEP_THREADS / 32;
 
     // ---- tile decode: binary search of blockIdx.x in the descending-band prefix ----
     const int tile = blockIdx.x;
-    int lo = 0, hi = P.nbands;  // tile_start[lo] <= tile < tile_start[hi]
+    int lo = 0, hi = P.nbands;
     while (hi - lo > 1) {
         int mid = (lo + hi) >> 1;
         if (__ldg(P.tile_start + mid) <= tile) lo = mid; else hi = mid;
@@ -58,12 +131,71 @@ __global__ void __launch_bounds__(SWEEP_THREADS, TJ_MINB) sweep_kernel(const __g
     const int band = P.nbands - 1 - lo;
     const int cb = tile - __ldg(P.tile_start + lo);
     const int a = band * R;
-    const int c = a + cb * SWEEP_THREADS + (int)threadIdx.x;
-    const int s = a + c;
-    const int s_min = s - (int)(threadIdx.x & 31);  // warp-uniform: smallest s of the warp
+    const int lane = (int)(threadIdx.x & 31), warp = (int)(threadIdx.x >> 5);
+    const int cw = a + cb * SWEEP_THREADS + warp * 32;   // first column of the warp
+    const int c = cw + lane;
+    const int sw = a + cw;                               // smallest s of the warp
 
     // a warp whose columns all lie beyond lmax has nothing to store
-    if (s_min - a - (R - 1) > P.lmax) return;
+    if (cw - (R - 1) > P.lmax) return;
+
+    double *const wbuf = reinterpret_cast<double *>(smem_raw) + warp * (NBUF * L::BUFD);
+    const uint32_t wbuf_s = smem_u32(wbuf);
+    const uint32_t bar_s = smem_u32(smem_raw) + (uint32_t)(NWARP * NBUF * L::BUFD) * 8u + (uint32_t)warp * (NBUF * 8u);
+    if (lane == 0) {
+#pragma unroll
+        for (int b = 0; b < NBUF; ++b) mbar_init(bar_s + 8u * b, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncwarp();
+
+    // ---- the warp's walk: odd-J stages first, then even-J stages ----
+    const int t_end = a + R - 1;   // last step any pair of the band can have
+    int tbo = sw - 1 - P.l3max;    // odd:  l3 = s-2t-1 <= l3max
+    tbo = tbo > 0 ? (tbo + 1) >> 1 : 0;
+    int tbe = sw - P.l3max;        // even: l3 = s-2t   <= l3max
+    tbe = tbe > 0 ? (tbe + 1) >> 1 : 0;
+    const int nso = (kEB && tbo <= t_end) ? (t_end - tbo + TS) / TS : 0;
+    const int nse = (kEven && tbe <= t_end) ? (t_end - tbe + TS) / TS : 0;
+    const int ntot = nso + nse;
+
+    // producer (lane 0): ask for every slice of global stage index q
+    auto issue = [&](int q) {
+        const int b = q % NBUF;
+        const uint32_t buf = wbuf_s + (uint32_t)(b * L::BUFD) * 8u;
+        const uint32_t bar = bar_s + 8u * b;
+        if (q < nso) {
+            const int t0 = tbo + q * TS, tl = t0 + TS - 1;
+            uint32_t bytes = slice_bytes(a - tl, TS) + slice_bytes(t0, TS) + slice_bytes(cw - R + 1 - tl, TS + 31) +
+                             slice_bytes(sw - tl, TS + 31) + 2 * slice_bytes(sw - 2 * tl - 1, 2 * (TS - 1) + 32);
+            mbar_expect_tx(bar, bytes);
+            slice(buf, L::OA, P.gA, a - tl, TS, bar);
+            slice(buf, L::OG, P.gB, t0, TS, bar);
+            slice(buf, L::OB, P.gA, cw - R + 1 - tl, TS + 31, bar);
+            slice(buf, L::OH, P.ginv, sw - tl, TS + 31, bar);
+            slice(buf, L::OW2, P.wpp, sw - 2 * tl - 1, 2 * (TS - 1) + 32, bar);
+            slice(buf, L::OU, P.u3, sw - 2 * tl - 1, 2 * (TS - 1) + 32, bar);
+        } else {
+            const int t0 = tbe + (q - nso) * TS, tl = t0 + TS - 1;
+            const int nwin = (kTT ? 1 : 0) + (kTE ? 1 : 0) + (kEE ? 1 : 0) + (kA2 ? 1 : 0);
+            uint32_t bytes = slice_bytes(a - tl, TS) + slice_bytes(t0, TS) + slice_bytes(cw - R + 1 - tl, TS + 31) +
+                             slice_bytes(sw - tl, TS + 31) + nwin * slice_bytes(sw - 2 * tl, 2 * (TS - 1) + 32);
+            mbar_expect_tx(bar, bytes);
+            slice(buf, L::OA, P.g, a - tl, TS, bar);
+            slice(buf, L::OG, P.g, t0, TS, bar);
+            slice(buf, L::OB, P.g, cw - R + 1 - tl, TS + 31, bar);
+            slice(buf, L::OH, P.h, sw - tl, TS + 31, bar);
+            if (kTT) slice(buf, L::OW0, P.wtt, sw - 2 * tl, 2 * (TS - 1) + 32, bar);
+            if (kTE) slice(buf, L::OW1, P.wtp, sw - 2 * tl, 2 * (TS - 1) + 32, bar);
+            if (kEE) slice(buf, L::OW2, P.wpp, sw - 2 * tl, 2 * (TS - 1) + 32, bar);
+            if (kA2) slice(buf, L::OU, P.u3, sw - 2 * tl, 2 * (TS - 1) + 32, bar);
+        }
+    };
+    if (lane == 0) {
+#pragma unroll
+        for (int q = 0; q < NBUF; ++q)
+            if (q < ntot) issue(q);
+    }
 
     // ---- per-pair constants ----
     double c12[R], kk[R];
@@ -77,56 +209,64 @@ __global__ void __launch_bounds__(SWEEP_THREADS, TJ_MINB) sweep_kernel(const __g
         }
     }
 
-    const int t_end = a + R - 1;  // last step any pair of the band can have (t <= min(l1,l2) <= l1)
+    int q = 0;   // global stage index
 
     // =========================== odd-J branch: EB ===========================
     if (kEB) {
         double acc[R];
 #pragma unroll
         for (int i = 0; i < R; ++i) acc[i] = 0.0;
-        // l3 = s-2t-1 <= l3max  <=>  t >= (s-1-l3max)/2
-        int tb = s_min - 1 - P.l3max;
-        tb = tb > 0 ? (tb + 1) >> 1 : 0;
-        if (tb <= t_end) {
-            const int nblk = (t_end - tb + R) / R;
+        if (nso > 0) {
             double wa[R], wb[R];
-            const double *pa = P.gA + (a - tb);
-            const double *pb = P.gA + (c - R + 1 - tb);
-            const double *ph = P.ginv + (s - tb);
-            const double *pg = P.gB + tb;
-            const double *pw = P.wpp + (s - 2 * tb - 1);
-            const double *pu = P.u3 + (s - 2 * tb - 1);
+            {   // ring start-up straight from global memory (once per warp)
+                const double *pa = P.gA + (a - tbo);
+                const double *pb = P.gA + (c - R + 1 - tbo);
 #pragma unroll
-            for (int k = 1; k < R; ++k) wa[k] = ldg(pa + k);                       // G[k] = gA[a-t0+k]
+                for (int k = 1; k < R; ++k) wa[k] = __ldg(pa + k);
 #pragma unroll
-            for (int i = 0; i < R - 1; ++i) wb[(R - i) % R] = ldg(pb + (R - 1 - i));  // H[-i] = gA[c-t0-i]
-            // software pipeline: the raw table values of substep u+1 are loaded while substep u computes
-            double xa = ldg(pa), xb = ldg(pb), xh = ldg(ph), xg = ldg(pg), xw = ldg(pw), xu = ldg(pu);
-            for (int blk = 0; blk < nblk; ++blk) {
+                for (int i = 0; i < R - 1; ++i) wb[(R - i) % R] = __ldg(pb + (R - 1 - i));
+            }
+            // consumer offsets: parity of each slice's first index is the same in every stage (TS even)
+            const int tl0 = tbo + TS - 1;
+            const int oa = L::OA + PAD + ((a - tl0) & 1) + (TS - 1);
+            const int og = L::OG + PAD + (tbo & 1);
+            const int ob = L::OB + PAD + ((cw - R + 1 - tl0) & 1) + (TS - 1) + lane;
+            const int oh = L::OH + PAD + ((sw - tl0) & 1) + (TS - 1) + lane;
+            const int ow = PAD + ((sw - 2 * tl0 - 1) & 1) + 2 * (TS - 1) + lane;
+            for (int k = 0; k < nso; ++k, ++q) {
+                const int b = q % NBUF;
+                mbar_wait(bar_s + 8u * b, (uint32_t)((q / NBUF) & 1));
+                const double *sb = wbuf + b * L::BUFD;
+                const double *pa = sb + oa, *pg = sb + og, *pb = sb + ob, *ph = sb + oh;
+                const double *pw = sb + L::OW2 + ow, *pu = sb + L::OU + ow;
+                double xa = pa[0], xb = pb[0], xh = ph[0], xg = pg[0], xw = pw[0], xu = pu[0];
+#pragma unroll 1
+                for (int blk = 0; blk < TS / R; ++blk) {
 #pragma unroll
-                for (int u = 0; u < R; ++u) {
-                    wa[(R - u) % R] = xa;
-                    wb[(R + 1 - u) % R] = xb;
-                    const double hg = __dmul_rn(xh, xg);
-                    const double q3 = __dmul_rn(xw, hg);
-                    const double c3 = xu;
-                    xa = ldg(pa - (u + 1)); xb = ldg(pb - (u + 1)); xh = ldg(ph - (u + 1)); xg = ldg(pg + (u + 1));
-                    xw = ldg(pw - 2 * (u + 1)); xu = ldg(pu - 2 * (u + 1));
-                    // op-major order: consecutive FP64 instructions share c3 / q3 in one operand slot, so
-                    // the register-file reuse cache serves it and no instruction needs 3 bank reads
-                    double r[R], e[R];
+                    for (int u = 0; u < R; ++u) {
+                        wa[(R - u) % R] = xa;
+                        wb[(R + 1 - u) % R] = xb;
+                        const double hg = __dmul_rn(xh, xg);
+                        const double q3 = __dmul_rn(xw, hg);
+                        const double c3 = xu;
+                        xa = pa[-(u + 1)]; xb = pb[-(u + 1)]; xh = ph[-(u + 1)]; xg = pg[u + 1];
+                        xw = pw[-2 * (u + 1)]; xu = pu[-2 * (u + 1)];
+                        double r[R], e[R];
 #pragma unroll
-                    for (int i = 0; i < R; ++i) r[i] = __dmul_rn(wa[(i - u + R) % R], wb[(2 * R - i - u) % R]);
+                        for (int i = 0; i < R; ++i) r[i] = __dmul_rn(wa[(i - u + R) % R], wb[(2 * R - i - u) % R]);
 #pragma unroll
-                    for (int i = 0; i < R; ++i) e[i] = __dsub_rn(c3, c12[i]);
+                        for (int i = 0; i < R; ++i) e[i] = __dsub_rn(c3, c12[i]);
 #pragma unroll
-                    for (int i = 0; i < R; ++i) r[i] = __dmul_rn(r[i], e[i]);
+                        for (int i = 0; i < R; ++i) r[i] = __dmul_rn(r[i], e[i]);
 #pragma unroll
-                    for (int i = 0; i < R; ++i) r[i] = __dmul_rn(r[i], e[i]);
+                        for (int i = 0; i < R; ++i) r[i] = __dmul_rn(r[i], e[i]);
 #pragma unroll
-                    for (int i = 0; i < R; ++i) acc[i] = __fma_rn(r[i], q3, acc[i]);
+                        for (int i = 0; i < R; ++i) acc[i] = __fma_rn(r[i], q3, acc[i]);
+                    }
+                    pa -= R; pb -= R; ph -= R; pg += R; pw -= 2 * R; pu -= 2 * R;
                 }
-                pa -= R; pb -= R; ph -= R; pg += R; pw -= 2 * R; pu -= 2 * R;
+                __syncwarp();
+                if (lane == 0 && q + NBUF < ntot) issue(q + NBUF);
             }
         }
         // epilogue: Xi_EB = S_EB / (4 D)
@@ -154,74 +294,108 @@ __global__ void __launch_bounds__(SWEEP_THREADS, TJ_MINB) sweep_kernel(const __g
 #pragma unroll
             for (int i = 0; i < R; ++i) c12[i] += 1.0;   // even branch: d1 = d+1 = u3 - (u1+u2-1)
         }
-        // l3 = s-2t <= l3max  <=>  t >= (s-l3max)/2
-        int tb = s_min - P.l3max;
-        tb = tb > 0 ? (tb + 1) >> 1 : 0;
-        if (tb <= t_end) {
-            const int nblk = (t_end - tb + R) / R;
+        if (nse > 0) {
             double wa[R], wb[R];
-            const double *pa = P.g + (a - tb);
-            const double *pb = P.g + (c - R + 1 - tb);
-            const double *ph = P.h + (s - tb);
-            const double *pg = P.g + tb;
-            const double *pwtt = P.wtt + (s - 2 * tb);
-            const double *pwtp = P.wtp + (s - 2 * tb);
-            const double *pwpp = P.wpp + (s - 2 * tb);
-            const double *pu = P.u3 + (s - 2 * tb);
+            {
+                const double *pa = P.g + (a - tbe);
+                const double *pb = P.g + (c - R + 1 - tbe);
 #pragma unroll
-            for (int k = 1; k < R; ++k) wa[k] = ldg(pa + k);
+                for (int k = 1; k < R; ++k) wa[k] = __ldg(pa + k);
 #pragma unroll
-            for (int i = 0; i < R - 1; ++i) wb[(R - i) % R] = ldg(pb + (R - 1 - i));
-            double xa = ldg(pa), xb = ldg(pb), xh = ldg(ph), xg = ldg(pg);
-            double xtt = kTT ? ldg(pwtt) : 0.0, xtp = kTE ? ldg(pwtp) : 0.0, xpp = kEE ? ldg(pwpp) : 0.0;
-            double xu = kA2 ? ldg(pu) : 0.0;
-            for (int blk = 0; blk < nblk; ++blk) {
+                for (int i = 0; i < R - 1; ++i) wb[(R - i) % R] = __ldg(pb + (R - 1 - i));
+            }
+            // PIPE: products of step t are accumulated at the start of step t+1 (see the loop body)
+            double rA[kTE ? R : 1], rAA[kEE ? R : 1], p1 = 0.0, p2 = 0.0;
 #pragma unroll
-                for (int u = 0; u < R; ++u) {
-                    wa[(R - u) % R] = xa;
-                    wb[(R + 1 - u) % R] = xb;
-                    const double hg = __dmul_rn(xh, xg);
-                    double q0 = 0.0, q1 = 0.0, q2 = 0.0;
-                    if (kTT) q0 = __dmul_rn(xtt, hg);
-                    if (kTE) q1 = __dmul_rn(xtp, hg);
-                    if (kEE) q2 = __dmul_rn(xpp, hg);
-                    const double c3 = xu;
-                    xa = ldg(pa - (u + 1)); xb = ldg(pb - (u + 1)); xh = ldg(ph - (u + 1)); xg = ldg(pg + (u + 1));
-                    if (kTT) xtt = ldg(pwtt - 2 * (u + 1));
-                    if (kTE) xtp = ldg(pwtp - 2 * (u + 1));
-                    if (kEE) xpp = ldg(pwpp - 2 * (u + 1));
-                    if (kA2) xu = ldg(pu - 2 * (u + 1));
-                    // op-major order (see the odd branch): q0/q1/q2/c3 stay in the operand reuse cache
-                    double r[R], A2[kA2 ? R : 1];
+            for (int i = 0; i < R; ++i) { if (kTE) rA[i] = 0.0; if (kEE) rAA[i] = 0.0; }
+            const int tl0 = tbe + TS - 1;
+            const int oa = L::OA + PAD + ((a - tl0) & 1) + (TS - 1);
+            const int og = L::OG + PAD + (tbe & 1);
+            const int ob = L::OB + PAD + ((cw - R + 1 - tl0) & 1) + (TS - 1) + lane;
+            const int oh = L::OH + PAD + ((sw - tl0) & 1) + (TS - 1) + lane;
+            const int ow = PAD + ((sw - 2 * tl0) & 1) + 2 * (TS - 1) + lane;
+            for (int k = 0; k < nse; ++k, ++q) {
+                const int b = q % NBUF;
+                mbar_wait(bar_s + 8u * b, (uint32_t)((q / NBUF) & 1));
+                const double *sb = wbuf + b * L::BUFD;
+                const double *pa = sb + oa, *pg = sb + og, *pb = sb + ob, *ph = sb + oh;
+                const double *pwtt = sb + L::OW0 + ow, *pwtp = sb + L::OW1 + ow, *pwpp = sb + L::OW2 + ow;
+                const double *pu = sb + L::OU + ow;
+                double xa = pa[0], xb = pb[0], xh = ph[0], xg = pg[0];
+                double xtt = kTT ? pwtt[0] : 0.0, xtp = kTE ? pwtp[0] : 0.0, xpp = kEE ? pwpp[0] : 0.0;
+                double xu = kA2 ? pu[0] : 0.0;
+#pragma unroll 1
+                for (int blk = 0; blk < TS / R; ++blk) {
 #pragma unroll
-                    for (int i = 0; i < R; ++i) r[i] = __dmul_rn(wa[(i - u + R) % R], wb[(2 * R - i - u) % R]);
-                    if (kA2) {
-#pragma unroll
-                        for (int i = 0; i < R; ++i) A2[i] = __dsub_rn(c3, c12[i]);
-                    }
-                    if (kTT) {
-#pragma unroll
-                        for (int i = 0; i < R; ++i) att[i] = __fma_rn(r[i], q0, att[i]);
-                    }
-                    if (kA2) {
-#pragma unroll
-                        for (int i = 0; i < R; ++i) A2[i] = __fma_rn(A2[i], A2[i], -kk[i]);
-#pragma unroll
-                        for (int i = 0; i < R; ++i) r[i] = __dmul_rn(r[i], A2[i]);
+                    for (int u = 0; u < R; ++u) {
+                        wa[(R - u) % R] = xa;
+                        wb[(R + 1 - u) % R] = xb;
+                        const double hg = __dmul_rn(xh, xg);
+                        double q0 = 0.0, q1 = 0.0, q2 = 0.0;
+                        if (kTT) q0 = __dmul_rn(xtt, hg);
+                        if (kTE) q1 = __dmul_rn(xtp, hg);
+                        if (kEE) q2 = __dmul_rn(xpp, hg);
+                        const double c3 = xu;
+                        xa = pa[-(u + 1)]; xb = pb[-(u + 1)]; xh = ph[-(u + 1)]; xg = pg[u + 1];
+                        if (kTT) xtt = pwtt[-2 * (u + 1)];
+                        if (kTE) xtp = pwtp[-2 * (u + 1)];
+                        if (kEE) xpp = pwpp[-2 * (u + 1)];
+                        if (kA2) xu = pu[-2 * (u + 1)];
+                        if (PIPE) {
+                        // accumulate the PREVIOUS step's products first (their inputs are long ready, so the
+                        // 8 FMAs of one window issue back to back and share q through the operand reuse cache)
                         if (kTE) {
 #pragma unroll
-                            for (int i = 0; i < R; ++i) ate[i] = __fma_rn(r[i], q1, ate[i]);
+                            for (int i = 0; i < R; ++i) ate[i] = __fma_rn(rA[i], p1, ate[i]);
                         }
                         if (kEE) {
 #pragma unroll
-                            for (int i = 0; i < R; ++i) r[i] = __dmul_rn(r[i], A2[i]);
+                            for (int i = 0; i < R; ++i) aee[i] = __fma_rn(rAA[i], p2, aee[i]);
+                        }
+                        p1 = q1; p2 = q2;
+                        }
+                        double r[R], A2[kA2 ? R : 1];
 #pragma unroll
-                            for (int i = 0; i < R; ++i) aee[i] = __fma_rn(r[i], q2, aee[i]);
+                        for (int i = 0; i < R; ++i) r[i] = __dmul_rn(wa[(i - u + R) % R], wb[(2 * R - i - u) % R]);
+                        if (kTT) {
+#pragma unroll
+                            for (int i = 0; i < R; ++i) att[i] = __fma_rn(r[i], q0, att[i]);
+                        }
+                        if (kA2) {
+#pragma unroll
+                            for (int i = 0; i < R; ++i) A2[i] = __dsub_rn(c3, c12[i]);
+#pragma unroll
+                            for (int i = 0; i < R; ++i) A2[i] = __fma_rn(A2[i], A2[i], -kk[i]);
+#pragma unroll
+                            for (int i = 0; i < R; ++i) rA[i] = __dmul_rn(r[i], A2[i]);
+                            if (kEE) {
+#pragma unroll
+                                for (int i = 0; i < R; ++i) rAA[i] = __dmul_rn(rA[i], A2[i]);
+                            }
+                        }
+                        if (!PIPE) {
+                        if (kTE) {
+#pragma unroll
+                            for (int i = 0; i < R; ++i) ate[i] = __fma_rn(rA[i], q1, ate[i]);
+                        }
+                        if (kEE) {
+#pragma unroll
+                            for (int i = 0; i < R; ++i) aee[i] = __fma_rn(rAA[i], q2, aee[i]);
+                        }
                         }
                     }
+                    pa -= R; pb -= R; ph -= R; pg += R;
+                    pwtt -= 2 * R; pwtp -= 2 * R; pwpp -= 2 * R; pu -= 2 * R;
                 }
-                pa -= R; pb -= R; ph -= R; pg += R;
-                pwtt -= 2 * R; pwtp -= 2 * R; pwpp -= 2 * R; pu -= 2 * R;
+                __syncwarp();
+                if (lane == 0 && q + NBUF < ntot) issue(q + NBUF);
+            }
+            if (PIPE) {
+#pragma unroll
+            for (int i = 0; i < R; ++i) {   // the last step's products
+                if (kTE) ate[i] = __fma_rn(rA[i], p1, ate[i]);
+                if (kEE) aee[i] = __fma_rn(rAA[i], p2, aee[i]);
+            }
             }
         }
         // epilogue: Xi_TT = S_TT; Xi_TE = S_TE/(2 sqrt D); Xi_EE = S_EE/(4 D)
@@ -242,22 +416,48 @@ __global__ void __launch_bounds__(SWEEP_THREADS, TJ_MINB) sweep_kernel(const __g
     }
 }
 
-template <int R, int MASK>
+template <int R, int MASK, int TS, int MINB, bool PIPE>
 cudaError_t launch_one(const SweepParams &P, int total_tiles, cudaStream_t st)
 {
     if (total_tiles <= 0) return cudaSuccess;
-    sweep_kernel<R, MASK><<<total_tiles, SWEEP_THREADS, 0, st>>>(P);
+    constexpr int NWARP = SWEEP_THREADS / 32;
+    constexpr size_t smem = (size_t)NWARP * NBUF * Lay<TS>::BUFD * 8 + (size_t)NWARP * NBUF * 8;
+    static bool attr_set = false;   // per instantiation
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(sweep_tma_kernel<R, MASK, TS, MINB, PIPE>,
+                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+    }
+    sweep_tma_kernel<R, MASK, TS, MINB, PIPE><<<total_tiles, SWEEP_THREADS, smem, st>>>(P);
     return cudaGetLastError();
 }
 
 }  // namespace
 
+// Geometry per request: dense sweeps are long (up to lmax steps per pair), so the per-step
+// overhead (prefactors, table reads) is spread over R = 12 pairs at 2 CTAs/SM with stages of 48 steps;
+// band-limited sweeps have <= lcut/2+1 steps per pair, so they keep R = 8 and short stages of 32 steps.
+int sweep_R(int mask, bool banded)
+{
+    if (mask == M_TT) return R_TT;
+    return banded ? R_POL_BAND : R_POL;
+}
+
 cudaError_t launch_sweep(const SweepParams &P, int mask, int total_tiles, cudaStream_t st)
 {
+    constexpr int POL = M_TE | M_EE | M_EB, ALL = M_TT | POL;
+    const bool banded = P.lcut >= 0;
     switch (mask) {
-        case M_TT: return launch_one<R_TT, M_TT>(P, total_tiles, st);
-        case M_TE | M_EE | M_EB: return launch_one<R_POL, M_TE | M_EE | M_EB>(P, total_tiles, st);
-        case M_TT | M_TE | M_EE | M_EB: return launch_one<R_POL, M_TT | M_TE | M_EE | M_EB>(P, total_tiles, st);
+        case M_TT:
+            return banded ? launch_one<R_TT, M_TT, 32, 3, false>(P, total_tiles, st)
+                          : launch_one<R_TT, M_TT, 48, 3, false>(P, total_tiles, st);
+        case POL:
+            return banded ? launch_one<R_POL_BAND, POL, 32, 3, false>(P, total_tiles, st)
+                          : launch_one<R_POL, POL, 48, 2, true>(P, total_tiles, st);
+        case ALL:
+            return banded ? launch_one<R_POL_BAND, ALL, 32, 3, false>(P, total_tiles, st)
+                          : launch_one<R_POL, ALL, 48, 2, true>(P, total_tiles, st);
         default: return cudaErrorInvalidValue;
     }
 }
