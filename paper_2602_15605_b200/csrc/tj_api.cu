@@ -64,9 +64,23 @@ int total_tiles(int lmax, int l3max, int R, bool banded)
     return n > 0x7fffffffLL ? -1 : (int)n;
 }
 
+// State of one coupling call between its pieces (coupling_begin / _sweep / _write / _end, below).
+struct Call {
+    const Tables *T = nullptr;
+    bool banded = false;
+    int lcut = -1, mask = 0, R = 0, l3max_eff = 0, nb = 0, ntiles = 0, ntile_w = 0;
+    long long N = 0, ld = 0;
+    double *TT = nullptr, *TE = nullptr, *ee = nullptr, *EB = nullptr, *bb_copy = nullptr;
+    unsigned char *scratch = nullptr;
+    double *wtt = nullptr, *wtp = nullptr, *wpp = nullptr;
+    int *tile_start = nullptr;
+};
+
 // One coupling call on device pointers.  lcut < 0: dense (l3max = handle's); else banded with l3 <= lcut.
 int run_coupling(const tj_tables *tables, int lcut, const double *d_Wtt, const double *d_Wtp, const double *d_Wpp,
                  int nW, double *d_TT, double *d_TE, double *d_EE, double *d_BB, double *d_EB, cudaStream_t st);
+int run_coupling_rows_to_host(const tj_tables *tables, const double *d_Wtt, const double *d_Wtp, const double *d_Wpp,
+                              int nW, double *const d_out[5], double *const h_out[5], cudaStream_t st);
 
 }  // namespace
 
@@ -220,11 +234,16 @@ int tj_coupling_host(const tj_tables *tables, int band, int nW_or_lcut, const do
         int j = 0;
         for (int k = 0; k < 5; ++k)
             if (ho[k] && !(k == 3 && bb_from_ee)) dop[k] = dout + per * (size_t)(j++);
-        rc = run_coupling(tables, lcut, dwp[0], dwp[1], dwp[2], nW, dop[0], dop[1], dop[2], dop[3], dop[4], st);
-        if (rc == TJ_OK) {
-            for (int k = 0; k < 5 && e == cudaSuccess; ++k) {
-                const double *src = (k == 3 && bb_from_ee) ? dop[2] : dop[k];
-                if (ho[k]) e = cudaMemcpyAsync(ho[k], src, sizeof(double) * per, cudaMemcpyDeviceToHost, st);
+        if (!band) {
+            // dense: sweep, writer and the copies to the host pipelined by row chunks
+            rc = run_coupling_rows_to_host(tables, dwp[0], dwp[1], dwp[2], nW, dop, ho, st);
+        } else {
+            rc = run_coupling(tables, lcut, dwp[0], dwp[1], dwp[2], nW, dop[0], dop[1], dop[2], dop[3], dop[4], st);
+            if (rc == TJ_OK) {
+                for (int k = 0; k < 5 && e == cudaSuccess; ++k) {
+                    const double *src = (k == 3 && bb_from_ee) ? dop[2] : dop[k];
+                    if (ho[k]) e = cudaMemcpyAsync(ho[k], src, sizeof(double) * per, cudaMemcpyDeviceToHost, st);
+                }
             }
         }
     }
@@ -329,85 +348,203 @@ int tj_launches_per_call(int which)
 
 namespace {
 
-int run_coupling(const tj_tables *tables, int lcut, const double *d_Wtt, const double *d_Wtp, const double *d_Wpp,
-                 int nW, double *d_TT, double *d_TE, double *d_EE, double *d_BB, double *d_EB, cudaStream_t st)
+// ---- one coupling call, in pieces (the host-buffer path launches the middle two per row chunk) -------------
+int coupling_begin(Call &C, const tj_tables *tables, int lcut, const double *d_Wtt, const double *d_Wtp,
+                   const double *d_Wpp, int nW, double *d_TT, double *d_TE, double *d_EE, double *d_BB, double *d_EB,
+                   cudaStream_t st)
 {
     const Tables &T = tables->T;
-    const bool banded = lcut >= 0;
+    C.T = &T;
+    C.banded = lcut >= 0;
+    C.lcut = lcut;
     // an output needs its window (TJ_EINVAL otherwise)
     if ((d_TT && !d_Wtt) || (d_TE && !d_Wtp) || ((d_EE || d_BB || d_EB) && !d_Wpp)) return TJ_EINVAL;
     if (!d_TT && !d_TE && !d_EE && !d_BB && !d_EB) return TJ_EINVAL;
     // EE target: EE if given, else BB takes the even spin-2 block directly
-    double *ee = d_EE ? d_EE : d_BB;
-    double *bb_copy = (d_EE && d_BB) ? d_BB : nullptr;
-
+    C.TT = d_TT; C.TE = d_TE; C.EB = d_EB;
+    C.ee = d_EE ? d_EE : d_BB;
+    C.bb_copy = (d_EE && d_BB) ? d_BB : nullptr;
     // smallest instantiated sweep that covers the request
-    int mask;
-    if (!d_TE && !ee && !d_EB) mask = M_TT;
-    else if (d_TT) mask = M_TT | M_TE | M_EE | M_EB;
-    else mask = M_TE | M_EE | M_EB;
-    const int R = sweep_R(mask, banded);
-    const int l3max_eff = banded ? lcut : T.l3max;
-    const long long N = (long long)T.lmax + 1;
-    const long long ld = banded ? (long long)(2 * lcut + 1) : N;
-    const size_t per = (size_t)N * (size_t)ld;
-
-    const int ntiles = total_tiles(T.lmax, l3max_eff, R, banded);
-    if (ntiles < 0) return TJ_EINVAL;
-    const int nb = num_bands(T.lmax, R);
+    if (!d_TE && !C.ee && !d_EB) C.mask = M_TT;
+    else if (d_TT) C.mask = M_TT | M_TE | M_EE | M_EB;
+    else C.mask = M_TE | M_EE | M_EB;
+    C.R = sweep_R(C.mask, C.banded);
+    C.l3max_eff = C.banded ? lcut : T.l3max;
+    C.N = (long long)T.lmax + 1;
+    C.ld = C.banded ? (long long)(2 * lcut + 1) : C.N;
+    C.ntiles = total_tiles(T.lmax, C.l3max_eff, C.R, C.banded);
+    if (C.ntiles < 0) return TJ_EINVAL;
+    C.nb = num_bands(T.lmax, C.R);
+    C.ntile_w = (int)((C.N + 31) / 32);
 
     // ---- stream-ordered scratch: 3 prefolded windows + tile prefix
     const size_t wbytes = sizeof(double) * 3 * (size_t)T.nl_alloc;
-    const size_t tbytes = sizeof(int) * (size_t)(nb + 1 + 1);
+    const size_t tbytes = sizeof(int) * (size_t)(C.nb + 1 + 1);
     const size_t tb_al = (tbytes + 15) & ~(size_t)15;
-    unsigned char *scratch = nullptr;
-    TJ_CUDA(cudaMallocAsync((void **)&scratch, wbytes + tb_al, st), "coupling/scratch");
-    double *wtt = (double *)scratch + GUARD_LO;
-    double *wtp = wtt + T.nl_alloc;
-    double *wpp = wtp + T.nl_alloc;
-    int *tile_start = (int *)(scratch + wbytes);
+    TJ_CUDA(cudaMallocAsync((void **)&C.scratch, wbytes + tb_al, st), "coupling/scratch");
+    C.wtt = (double *)C.scratch + GUARD_LO;
+    C.wtp = C.wtt + T.nl_alloc;
+    C.wpp = C.wtp + T.nl_alloc;
+    C.tile_start = (int *)(C.scratch + wbytes);
 
-    int rc = TJ_OK;
     prof_record(0, st);
-    cudaError_t e = launch_prepare(T, d_Wtt, d_Wtp, d_Wpp, nW, wtt, wtp, wpp, tile_start, R, l3max_eff, banded, st);
+    cudaError_t e = launch_prepare(T, d_Wtt, d_Wtp, d_Wpp, nW, C.wtt, C.wtp, C.wpp, C.tile_start, C.R, C.l3max_eff,
+                                   C.banded, st);
     prof_record(1, st);
-    if (e == cudaSuccess && banded) {
+    if (e == cudaSuccess && C.banded) {
         // slots of the band whose l2 falls outside 0..lmax (and everything the sweep does not own) are 0
+        const size_t per = (size_t)C.N * (size_t)C.ld;
         double *outs[5] = {d_TT, d_TE, d_EE, d_BB, d_EB};
         for (int k = 0; k < 5 && e == cudaSuccess; ++k)
             if (outs[k]) e = cudaMemsetAsync(outs[k], 0, sizeof(double) * per, st);
     }
+    if (e != cudaSuccess) { cudaFreeAsync(C.scratch, st); C.scratch = nullptr; return cuda_fail(e, "coupling/prepare"); }
+    return TJ_OK;
+}
+
+// tiles of the descending-band prefix that precede band b (= tiles of all bands > b); host copy of what
+// prepare_kernel writes to tile_start[]
+int tiles_above(const Call &C, int b)
+{
+    long long n = 0;
+    for (int k = C.nb - 1; k > b; --k) n += band_num_tiles(C.T->lmax, C.l3max_eff, C.R, k, C.banded);
+    return (int)n;
+}
+
+// sweep of the row bands [b0, b1)
+cudaError_t coupling_sweep(const Call &C, int b0, int b1, cudaStream_t st)
+{
+    const Tables &T = *C.T;
+    SweepParams P;
+    P.g = T.g; P.ginv = T.ginv; P.h = T.h; P.gA = T.gA; P.gB = T.gB; P.u3 = T.u3; P.isd = T.isd;
+    P.wtt = C.wtt; P.wtp = C.wtp; P.wpp = C.wpp;
+    // a block the instantiated sweep computes but the caller did not ask for has a NULL target and is not stored
+    P.TT = C.TT; P.TE = C.TE; P.EE = C.ee; P.EB = C.EB;
+    P.tile_start = C.tile_start;
+    P.lmax = T.lmax; P.l3max = C.l3max_eff; P.nbands = C.nb; P.lcut = C.banded ? C.lcut : -1; P.ld = C.ld;
+    const bool all = (b0 == 0 && b1 == C.nb);
+    P.tile_off = all ? 0 : tiles_above(C, b1 - 1);
+    const int n = all ? C.ntiles : tiles_above(C, b0 - 1) - P.tile_off;
+    return launch_sweep(P, C.mask, n, st);
+}
+
+// scale + mirror of the 32-row tile rows [I0, I1)
+cudaError_t coupling_write(const Call &C, int I0, int I1, cudaStream_t st)
+{
+    WriterParams W;
+    memset(&W, 0, sizeof(W));
+    int n = 0;
+    W.bb = nullptr; W.bb_src = -1;
+    if (C.TT) W.M[n++] = C.TT;
+    if (C.TE) W.M[n++] = C.TE;
+    if (C.ee) { if (C.bb_copy) { W.bb = C.bb_copy; W.bb_src = n; } W.M[n++] = C.ee; }
+    if (C.EB) W.M[n++] = C.EB;
+    W.nmat = n;
+    W.lmax = C.T->lmax; W.lcut = C.banded ? C.lcut : -1; W.ld = C.ld;
+    W.ntile = C.ntile_w;
+    const int tb = (C.lcut + 31) / 32 + 1;
+    W.tile_band = (C.banded && tb < W.ntile - 1) ? tb : W.ntile - 1;
+    W.I0 = I0; W.I1 = I1;
+    return launch_writer(W, st);
+}
+
+void coupling_end(Call &C, cudaStream_t st)
+{
+    if (C.scratch) cudaFreeAsync(C.scratch, st);
+    C.scratch = nullptr;
+}
+
+int run_coupling(const tj_tables *tables, int lcut, const double *d_Wtt, const double *d_Wtp, const double *d_Wpp,
+                 int nW, double *d_TT, double *d_TE, double *d_EE, double *d_BB, double *d_EB, cudaStream_t st)
+{
+    Call C;
+    int rc = coupling_begin(C, tables, lcut, d_Wtt, d_Wtp, d_Wpp, nW, d_TT, d_TE, d_EE, d_BB, d_EB, st);
+    if (rc != TJ_OK) return rc;
     prof_record(2, st);
-    if (e == cudaSuccess) {
-        SweepParams P;
-        P.g = T.g; P.ginv = T.ginv; P.h = T.h; P.gA = T.gA; P.gB = T.gB; P.u3 = T.u3; P.isd = T.isd;
-        P.wtt = wtt; P.wtp = wtp; P.wpp = wpp;
-        // a block the instantiated sweep computes but the caller did not ask for has a NULL target
-        // and is not stored
-        P.TT = d_TT; P.TE = d_TE; P.EE = ee; P.EB = d_EB;
-        P.tile_start = tile_start;
-        P.lmax = T.lmax; P.l3max = l3max_eff; P.nbands = nb; P.lcut = banded ? lcut : -1; P.ld = ld;
-        e = launch_sweep(P, mask, ntiles, st);
-    }
+    cudaError_t e = coupling_sweep(C, 0, C.nb, st);
     prof_record(3, st);
-    if (e == cudaSuccess) {
-        WriterParams W;
-        memset(&W, 0, sizeof(W));
-        int n = 0;
-        W.bb = nullptr; W.bb_src = -1;
-        if (d_TT) W.M[n++] = d_TT;
-        if (d_TE) W.M[n++] = d_TE;
-        if (ee) { if (bb_copy) { W.bb = bb_copy; W.bb_src = n; } W.M[n++] = ee; }
-        if (d_EB) W.M[n++] = d_EB;
-        W.nmat = n;
-        W.lmax = T.lmax; W.lcut = banded ? lcut : -1; W.ld = ld;
-        W.ntile = (int)((N + 31) / 32);
-        W.tile_band = banded ? ((lcut + 31) / 32 + 1 < W.ntile - 1 ? (lcut + 31) / 32 + 1 : W.ntile - 1) : W.ntile - 1;
-        e = launch_writer(W, st);
-    }
+    if (e == cudaSuccess) e = coupling_write(C, 0, C.ntile_w, st);
     prof_record(4, st);
     if (e != cudaSuccess) rc = cuda_fail(e, "coupling");
-    cudaFreeAsync(scratch, st);
+    coupling_end(C, st);
+    return rc;
+}
+// ---- dense call with HOST outputs, pipelined by row chunks ------------------------------------------------
+// Full row l1 of a matrix is final once (i) the sweep and writer of its own row band have run (upper part
+// and diagonal) and (ii) the writers of every band above it have run (they store the mirrored lower part).
+// So the bands are processed in ASCENDING row chunks; after chunk k the rows of chunk k are copied to the
+// host while chunk k+1 is computed.  Successive chunks alternate between two compute streams so that one
+// chunk's last CTAs overlap the next chunk's first ones; within a chunk the tiles keep the descending
+// (largest-first) order.  The chunks shrink towards the last rows, where a row is cheap to compute but as
+// large to copy as any other (the exposed tail is the copy of the last chunk).
+struct HostPipe {
+    cudaStream_t comp[2] = {nullptr, nullptr}, copy = nullptr;
+    bool have = false;
+};
+thread_local HostPipe g_pipe;
+
+int run_coupling_rows_to_host(const tj_tables *tables, const double *d_Wtt, const double *d_Wtp, const double *d_Wpp,
+                              int nW, double *const d_out[5], double *const h_out[5], cudaStream_t st)
+{
+    static const double kFrac[] = {0.25, 0.40, 0.50, 0.58, 0.65, 0.71, 0.76, 0.80, 0.84, 0.87, 0.90, 0.925, 0.95, 0.975, 1.0};
+    constexpr int KMAX = (int)(sizeof(kFrac) / sizeof(kFrac[0]));
+    if (!g_pipe.have) {
+        for (int k = 0; k < 2; ++k) TJ_CUDA(cudaStreamCreateWithFlags(&g_pipe.comp[k], cudaStreamNonBlocking), "host pipe");
+        TJ_CUDA(cudaStreamCreateWithFlags(&g_pipe.copy, cudaStreamNonBlocking), "host pipe");
+        g_pipe.have = true;
+    }
+    Call C;
+    int rc = coupling_begin(C, tables, -1, d_Wtt, d_Wtp, d_Wpp, nW, d_out[0], d_out[1], d_out[2], d_out[3], d_out[4], st);
+    if (rc != TJ_OK) return rc;
+    // chunk boundaries: multiples of lcm(R, 32) rows (whole row bands of the sweep, whole tile rows of the writer)
+    int L = C.R;
+    while (L % 32) L += C.R;
+    int bound[KMAX + 1];
+    int nchunk = 0;
+    bound[0] = 0;
+    for (int k = 0; k < KMAX; ++k) {
+        long long r = (k == KMAX - 1) ? C.N : (long long)(kFrac[k] * (double)C.N) / L * L;
+        if (r > bound[nchunk]) bound[++nchunk] = (int)r;
+    }
+    cudaEvent_t ev[KMAX + 2];
+    int nev = 0;
+    cudaError_t e = cudaSuccess;
+    for (int k = 0; k < nchunk + 2 && e == cudaSuccess; ++k) {
+        e = cudaEventCreateWithFlags(&ev[k], cudaEventDisableTiming);
+        if (e == cudaSuccess) ++nev;
+    }
+    cudaEvent_t fork = ev[nchunk], join = ev[nchunk + 1];
+    if (e == cudaSuccess) e = cudaEventRecord(fork, st);
+    for (int k = 0; k < 2 && e == cudaSuccess; ++k) e = cudaStreamWaitEvent(g_pipe.comp[k], fork, 0);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(g_pipe.copy, fork, 0);
+    for (int k = 0; k < nchunk && e == cudaSuccess; ++k) {
+        const int r0 = bound[k], r1 = bound[k + 1];
+        cudaStream_t cs = g_pipe.comp[k & 1];
+        const int b1 = (r1 == C.N) ? C.nb : r1 / C.R;
+        const int I1 = (r1 == C.N) ? C.ntile_w : r1 / 32;
+        e = coupling_sweep(C, r0 / C.R, b1, cs);
+        if (e == cudaSuccess) e = coupling_write(C, r0 / 32, I1, cs);
+        if (e == cudaSuccess) e = cudaEventRecord(ev[k], cs);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(g_pipe.copy, ev[k], 0);
+        if (e == cudaSuccess && k > 0) e = cudaStreamWaitEvent(g_pipe.copy, ev[k - 1], 0);
+        const size_t off = (size_t)r0 * (size_t)C.N, bytes = sizeof(double) * (size_t)(r1 - r0) * (size_t)C.N;
+        for (int m = 0; m < 5 && e == cudaSuccess; ++m) {
+            if (!h_out[m]) continue;
+            const double *src = d_out[m] ? d_out[m] : d_out[2];   // BB without its own device matrix: the EE rows
+            e = cudaMemcpyAsync(h_out[m] + off, src + off, bytes, cudaMemcpyDeviceToHost, g_pipe.copy);
+        }
+    }
+    // join: the caller's stream continues after everything issued above
+    if (nev == nchunk + 2) {
+        for (int k = 0; k < 2; ++k)
+            if (cudaEventRecord(join, g_pipe.comp[k]) == cudaSuccess) cudaStreamWaitEvent(st, join, 0);
+        if (cudaEventRecord(join, g_pipe.copy) == cudaSuccess) cudaStreamWaitEvent(st, join, 0);
+    } else {
+        cudaDeviceSynchronize();
+    }
+    if (e != cudaSuccess) rc = cuda_fail(e, "coupling/host pipeline");
+    coupling_end(C, st);
+    for (int k = 0; k < nev; ++k) cudaEventDestroy(ev[k]);
     return rc;
 }
 

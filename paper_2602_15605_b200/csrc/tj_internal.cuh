@@ -64,6 +64,7 @@ struct SweepParams {
     double *TT, *TE, *EE, *EB;      // raw Xi, upper triangle (dense: [l1*ld+l2]; band: [l1*ld + l2-l1+lcut])
     const int *tile_start;          // [nbands+1] exclusive prefix of tiles per band, bands in DESCENDING order
     int lmax, l3max, nbands, lcut;  // lcut < 0: dense storage
+    int tile_off;                   // first tile of this launch in the descending-band prefix (row-chunked launches)
     long long ld;                   // row stride of the outputs
 };
 
@@ -76,6 +77,7 @@ struct WriterParams {
     long long ld;
     int ntile;                      // tiles per side (ceil((lmax+1)/32))
     int tile_band;                  // banded: tiles (I,J) with J-I <= tile_band
+    int I0, I1;                     // tile rows [I0, I1) of this launch (row-chunked launches; whole matrix: 0, ntile)
 };
 
 // kernels / launchers (defined in the .cu files)

@@ -122,7 +122,7 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB) sweep_tma_kernel(const __
     constexpr int NWARP = SWEEP_THREADS / 32;
 
     // ---- tile decode: binary search of blockIdx.x in the descending-band prefix ----
-    const int tile = blockIdx.x;
+    const int tile = (int)blockIdx.x + P.tile_off;
     int lo = 0, hi = P.nbands;
     while (hi - lo > 1) {
         int mid = (lo + hi) >> 1;

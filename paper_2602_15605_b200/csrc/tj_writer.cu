@@ -28,7 +28,7 @@ __global__ void __launch_bounds__(WT * WROWS) writer_kernel(const __grid_constan
 {
     __shared__ double tile[WT][WT + 1];
     // tile pair decode: blockIdx.x enumerates (I, dJ) with J = I + dJ
-    const int I = blockIdx.x / (P.tile_band + 1);
+    const int I = P.I0 + blockIdx.x / (P.tile_band + 1);
     const int J = I + blockIdx.x % (P.tile_band + 1);
     if (J >= P.ntile) return;
     const int m = blockIdx.y;
@@ -72,8 +72,8 @@ __global__ void __launch_bounds__(WT * WROWS) writer_kernel(const __grid_constan
 
 cudaError_t launch_writer(const WriterParams &P, cudaStream_t st)
 {
-    if (P.nmat <= 0) return cudaSuccess;
-    dim3 grid((unsigned)(P.ntile * (P.tile_band + 1)), (unsigned)P.nmat, 1);
+    if (P.nmat <= 0 || P.I1 <= P.I0) return cudaSuccess;
+    dim3 grid((unsigned)((P.I1 - P.I0) * (P.tile_band + 1)), (unsigned)P.nmat, 1);
     dim3 block(WT, WROWS, 1);
     writer_kernel<<<grid, block, 0, st>>>(P);
     return cudaGetLastError();

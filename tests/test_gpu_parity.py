@@ -285,6 +285,30 @@ def test_host_entry_point_matches_device_path():
     T.close()
 
 
+@pytest.mark.parametrize("lmax,keys", [(1500, BLOCKS), (1000, ("BB", "EB")), (777, ("TT",))])
+def test_host_pipeline_many_row_chunks_bitwise(lmax, keys):
+    """The host-buffer path runs sweep + writer + copies per row chunk on several streams; every chunking must
+    give bit-identical matrices to the single-launch device path (which the tests above hold against the oracle)."""
+    import torch
+    wl = windows.config(2, lmax=lmax)
+    T = binding.build_tables(wl.lmax)
+    dev = [torch.as_tensor(w).cuda() for w in (wl.Wtt, wl.Wtp, wl.Wpp)]
+    ref = binding.coupling_pol(T, *dev)
+    torch.cuda.synchronize()
+    N = wl.lmax + 1
+    out = {k: torch.full((N, N), np.nan, dtype=torch.float64).pin_memory() for k in keys}
+    hw = [torch.as_tensor(w).pin_memory() for w in (wl.Wtt, wl.Wtp, wl.Wpp)]
+    if keys == ("TT",):
+        binding.coupling_host(T, hw[0], None, None, out)
+    elif "TT" not in keys:
+        binding.coupling_host(T, None, None, hw[2], out)
+    else:
+        binding.coupling_host(T, *hw, out)
+    for k in keys:
+        assert np.array_equal(out[k].numpy(), ref[k].cpu().numpy()), k
+    T.close()
+
+
 # ---------------------------------------------------------------- T3 full-size configs, sampled
 def _sample_pairs(lmax, n, seed, band=None):
     rng = np.random.default_rng(seed)
