@@ -273,7 +273,7 @@ def main():
     nmirror = len(blocks) - (1 if "BB" in blocks else 0)
     writer_bytes = int(nmirror * 1.5 * N * width * 8 + (N * width * 8 if "BB" in blocks else 0))
     roofline = {
-        "bound": "alu", "kernel": "sweep_kernel<R=8,TT|TE|EE|EB>" if wl.pol else "sweep_kernel<R=16,TT>",
+        "bound": "alu", "kernel": ("sweep_tma_kernel<R=8,TS=32>" if wl.band else "sweep_tma_kernel<R=12,TT|TE|EE|EB,TS=48,PIPE>") if wl.pol else "sweep_tma_kernel<R=16,TT>",
         "achieved": achieved / 1e12, "peak": peak_instr / 1e12, "unit": "T FP64 thread-instr/s",
         "frac": achieved / peak_instr,
         # dram__bytes_read.sum + dram__bytes_write.sum of one sweep launch, from the ncu --set full capture
