@@ -166,6 +166,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json configs index (headline: 3)")
+    ap.add_argument("--nwin", type=int, default=1,
+                    help="window sets per step through tj_coupling_multi (default 1: the headline tj_coupling_pol step)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
@@ -211,11 +213,23 @@ def main():
     T = binding.build_tables(wl.lmax, None if not wl.band else 2 * wl.lmax)
     dW = [None if w is None else torch.as_tensor(w, dtype=torch.float64).cuda() for w in (wl.Wtt, wl.Wtp, wl.Wpp)]
     width = (2 * wl.l3max + 1) if wl.band else N
-    out = {k: torch.empty((N, width), dtype=torch.float64, device="cuda") for k in blocks}
+    nwin = max(1, args.nwin)
+    if nwin > 1:
+        # multi-window batching: nwin window sets of the same recipe, scaled copies of the
+        # seeded set (the throughput does not depend on the values); one tj_coupling_multi call per step
+        assert wl.pol and not wl.band, "--nwin needs a dense polarised config"
+        args.no_e2e = True
+        dW = [torch.stack([w * (1.0 + 0.01 * k) for k in range(nwin)]).contiguous() for w in dW]
+        terms *= nwin
+        out = {k: torch.empty((nwin, N, width), dtype=torch.float64, device="cuda") for k in blocks}
+    else:
+        out = {k: torch.empty((N, width), dtype=torch.float64, device="cuda") for k in blocks}
     flush = torch.empty(512 * 1024 * 1024 // 8, dtype=torch.float64, device="cuda")
 
     def step():
-        if wl.band:
+        if nwin > 1:
+            binding.coupling_multi(T, *dW, want=blocks, out=out)
+        elif wl.band:
             binding.coupling_band(T, wl.l3max, *dW, want=blocks, out=out)
         elif wl.pol:
             binding.coupling_pol(T, *dW, want=blocks, out=out)
@@ -264,6 +278,12 @@ def main():
     else:
         alg_instr = INSTR_EVEN_TT * E
         alg_flops = 3 * E
+    if nwin > 1:
+        # the per-kernel events cover the LAST sweep of the call (one pair of window sets, or a single set when
+        # nwin is odd); algorithmic work is counted as for the unbatched method: (8E+5O) per window set
+        last = 2 if nwin % 2 == 0 else 1
+        alg_instr *= last
+        alg_flops *= last
     peaks, peak_kind = _peaks()
     sm_max = float(clocks.get("sm_max_mhz") or peaks.get("sm_max_mhz", 1965.0))
     peak_instr = SM_COUNT * FP64_LANES_PER_SM * sm_max * 1e6          # thread-instr/s at max boost
@@ -273,7 +293,7 @@ def main():
     nmirror = len(blocks) - (1 if "BB" in blocks else 0)
     writer_bytes = int(nmirror * 1.5 * N * width * 8 + (N * width * 8 if "BB" in blocks else 0))
     roofline = {
-        "bound": "alu", "kernel": ("sweep_tma_kernel<R=8,TS=32>" if wl.band else "sweep_tma_kernel<R=12,TT|TE|EE|EB,TS=48,PIPE>") if wl.pol else "sweep_tma_kernel<R=16,TT>",
+        "bound": "alu", "kernel": "sweep_tma_kernel<R=8,TT|TE|EE|EB,TS=48,PIPE,NW=2>" if nwin > 1 and nwin % 2 == 0 else ("sweep_tma_kernel<R=8,TS=32>" if wl.band else "sweep_tma_kernel<R=12,TT|TE|EE|EB,TS=48,PIPE>") if wl.pol else "sweep_tma_kernel<R=16,TT>",
         "achieved": achieved / 1e12, "peak": peak_instr / 1e12, "unit": "T FP64 thread-instr/s",
         "frac": achieved / peak_instr,
         # dram__bytes_read.sum + dram__bytes_write.sum of one sweep launch, from the ncu --set full capture
@@ -324,13 +344,15 @@ def main():
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": total_ms / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": wl.name, "lmax": wl.lmax, "l3max": wl.l3max, "blocks": "+".join(blocks),
+            "config": {"workload": wl.name, "lmax": wl.lmax, "l3max": wl.l3max, "blocks": "+".join(blocks), "window_sets_per_step": nwin,
                        "terms_even": E, "terms_odd": O, "pairs_upper": P,
                        "pairs_per_s": world * P * args.steps / (total_ms * 1e-3),
                        "l2": "512 MB flush written between timed steps; each step also writes %.1f GB of output" % (bytes_out / 1e9),
                        "parallelism": "1 problem per GPU" if world > 1 else "single GPU"},
             "roofline": roofline, "cpu_baseline": cpu_baseline, "e2e": e2e,
-            "gpu_launches": binding.launches_per_call(1) * args.steps,
+            # a batched pair of window sets: 2 prepare + 1 sweep + 2 writer launches; a single set: 3
+            "gpu_launches": ((nwin // 2) * 5 + (nwin % 2) * 3) * args.steps if nwin > 1
+            else binding.launches_per_call(1) * args.steps,
             "clocks": clocks, "wall_s_timed_region": t_wall, "step_ms": step_ms,
             "context": {"paper_A100_TT_lmax1e4_s": 0.63, "paper_A100_EE_lmax1e4_s": 3.2,
                         "note": "paper numbers (PAPER.md:242) are another machine's: context, not the target"},

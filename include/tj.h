@@ -91,6 +91,21 @@ int tj_coupling_band(const tj_tables *tables, int lcut,
                      void *cuda_stream);
 
 /*
+ * tj_coupling_multi -- multi-window batching (one coupling matrix per
+ * map pair / frequency pair, all on the same (l1,l2,l3) geometry; covariance matrices use
+ * the same symbols with the spectrum of the squared mask as window).  nwin independent window SETS
+ * (W^TT, W^TP, W^PP) are swept together: the squared symbols of a term (Eq. 10 product, A, A^2) are formed
+ * once and each set adds only its own multiply-adds.  Results are those of nwin tj_coupling_pol calls
+ * (same arithmetic per entry, so they agree to the last bit).
+ *   Windows: [nwin][nW] row-major, nW = l3max+1.  Outputs: [nwin][(lmax+1)^2].  NULL rules as tj_coupling_pol;
+ *   requests for all of TT, TE, EE (or BB) and EB run two sets per sweep, other requests one set per sweep.
+ */
+int tj_coupling_multi(const tj_tables *tables, int nwin,
+                      const double *d_Wtt, const double *d_Wtp, const double *d_Wpp, int nW,
+                      double *d_TT, double *d_TE, double *d_EE, double *d_BB, double *d_EB,
+                      void *cuda_stream);
+
+/*
  * Host-buffer forms (the end-to-end path): same semantics, but every window and output is a HOST
  * pointer (h_*; pinned memory makes the copies asynchronous and fast, pageable memory also works).
  * The call allocates device scratch from the stream-ordered pool, copies the windows in, runs the same

@@ -18,7 +18,7 @@ TJ_OK, TJ_EINVAL, TJ_ENOMEM, TJ_ECUDA = 0, -1, -2, -3
 # every symbol include/tj.h declares (tests/test_abi.py checks the header against this and the .so)
 SYMBOLS = (
     "tj_build_tables", "tj_free_tables", "tj_tables_info", "tj_tables_copy",
-    "tj_coupling_tt", "tj_coupling_pol", "tj_coupling_band", "tj_coupling_host",
+    "tj_coupling_tt", "tj_coupling_pol", "tj_coupling_band", "tj_coupling_multi", "tj_coupling_host",
     "tj_l3_range", "tj_sweep_counts", "tj_fp64_probe", "tj_profile_enable", "tj_profile_get",
     "tj_launches_per_call", "tj_strerror",
 )
@@ -52,6 +52,7 @@ def load_library() -> ctypes.CDLL:
     L.tj_coupling_tt.argtypes = [vp, vp, ci, vp, vp]
     L.tj_coupling_pol.argtypes = [vp, vp, vp, vp, ci, vp, vp, vp, vp, vp, vp]
     L.tj_coupling_band.argtypes = [vp, ci, vp, vp, vp, vp, vp, vp, vp, vp, vp]
+    L.tj_coupling_multi.argtypes = [vp, ci, vp, vp, vp, ci, vp, vp, vp, vp, vp, vp]
     L.tj_coupling_host.argtypes = [vp, ci, ci, vp, vp, vp, vp, vp, vp, vp, vp, vp]
     L.tj_l3_range.argtypes = [ci, ci, ci, ci, ip, ip, ip]
     L.tj_sweep_counts.argtypes = [ci, ci, ci, ip, ip, ip, ip]
@@ -196,6 +197,24 @@ def coupling_band(tables: Tables, lcut: int, Wtt, Wtp, Wpp, want=_BLOCKS, out=No
     _check(load_library().tj_coupling_band(tables.handle, int(lcut), _dev_ptr(Wtt, lcut + 1, "Wtt"),
                                            _dev_ptr(Wtp, lcut + 1, "Wtp"), _dev_ptr(Wpp, lcut + 1, "Wpp"),
                                            *args, _stream_ptr(stream)), "tj_coupling_band")
+    return {k: out[k] for k in want}
+
+
+def coupling_multi(tables: Tables, Wtt, Wtp, Wpp, want=_BLOCKS, out=None, stream=None):
+    """tj_coupling_multi.  Windows: float64 CUDA tensors [nwin, l3max+1]; outputs [nwin, lmax+1, lmax+1]."""
+    import torch
+    N = tables.lmax + 1
+    nW = tables.l3max + 1
+    first = next(w for w in (Wtt, Wtp, Wpp) if w is not None)
+    nwin = int(first.shape[0])
+    out = {} if out is None else dict(out)
+    for k in want:
+        if k not in out:
+            out[k] = torch.empty((nwin, N, N), dtype=torch.float64, device=first.device)
+    args = [_dev_ptr(out.get(k) if k in want else None, nwin * N * N, k) for k in _BLOCKS]
+    _check(load_library().tj_coupling_multi(tables.handle, nwin, _dev_ptr(Wtt, nwin * nW, "Wtt"),
+                                            _dev_ptr(Wtp, nwin * nW, "Wtp"), _dev_ptr(Wpp, nwin * nW, "Wpp"), nW,
+                                            *args, _stream_ptr(stream)), "tj_coupling_multi")
     return {k: out[k] for k in want}
 
 

@@ -69,6 +69,8 @@ struct Call {
     const Tables *T = nullptr;
     bool banded = false;
     int lcut = -1, mask = 0, R = 0, l3max_eff = 0, nb = 0, ntiles = 0, ntile_w = 0;
+    int nw = 1;                     // window sets per sweep (tj_coupling_multi: 2)
+    int nW = 0;                     // entries per window
     long long N = 0, ld = 0;
     double *TT = nullptr, *TE = nullptr, *ee = nullptr, *EB = nullptr, *bb_copy = nullptr;
     unsigned char *scratch = nullptr;
@@ -78,7 +80,7 @@ struct Call {
 
 // One coupling call on device pointers.  lcut < 0: dense (l3max = handle's); else banded with l3 <= lcut.
 int run_coupling(const tj_tables *tables, int lcut, const double *d_Wtt, const double *d_Wtp, const double *d_Wpp,
-                 int nW, double *d_TT, double *d_TE, double *d_EE, double *d_BB, double *d_EB, cudaStream_t st);
+                 int nW, double *d_TT, double *d_TE, double *d_EE, double *d_BB, double *d_EB, cudaStream_t st, int nw = 1);
 int run_coupling_rows_to_host(const tj_tables *tables, const double *d_Wtt, const double *d_Wtp, const double *d_Wpp,
                               int nW, double *const d_out[5], double *const h_out[5], cudaStream_t st);
 
@@ -194,6 +196,28 @@ int tj_coupling_band(const tj_tables *tables, int lcut, const double *d_Wtt, con
     if (lcut < 0 || lcut > 2 * tables->T.lmax) return TJ_EINVAL;
     return run_coupling(tables, lcut, d_Wtt, d_Wtp, d_Wpp, lcut + 1, d_TT, d_TE, d_EE, d_BB, d_EB,
                         (cudaStream_t)cuda_stream);
+}
+
+int tj_coupling_multi(const tj_tables *tables, int nwin, const double *d_Wtt, const double *d_Wtp, const double *d_Wpp,
+                      int nW, double *d_TT, double *d_TE, double *d_EE, double *d_BB, double *d_EB, void *cuda_stream)
+{
+    if (!tables || nwin < 1) return TJ_EINVAL;
+    if (nW != tables->T.l3max + 1) return TJ_EINVAL;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t per = ((size_t)tables->T.lmax + 1) * ((size_t)tables->T.lmax + 1);
+    // the batched sweep is instantiated for the full set of blocks; any other request runs one window set at a time
+    const bool full = d_Wtt && d_Wtp && d_Wpp && d_TT && d_TE && (d_EE || d_BB) && d_EB;
+    int w = 0;
+    while (w < nwin) {
+        const int nw = (full && nwin - w >= 2) ? 2 : 1;
+        const size_t wi = (size_t)w * (size_t)nW, oi = (size_t)w * per;
+        int rc = run_coupling(tables, -1, d_Wtt ? d_Wtt + wi : nullptr, d_Wtp ? d_Wtp + wi : nullptr,
+                              d_Wpp ? d_Wpp + wi : nullptr, nW, d_TT ? d_TT + oi : nullptr, d_TE ? d_TE + oi : nullptr,
+                              d_EE ? d_EE + oi : nullptr, d_BB ? d_BB + oi : nullptr, d_EB ? d_EB + oi : nullptr, st, nw);
+        if (rc != TJ_OK) return rc;
+        w += nw;
+    }
+    return TJ_OK;
 }
 
 int tj_coupling_host(const tj_tables *tables, int band, int nW_or_lcut, const double *h_Wtt, const double *h_Wtp,
@@ -351,10 +375,12 @@ namespace {
 // ---- one coupling call, in pieces (the host-buffer path launches the middle two per row chunk) -------------
 int coupling_begin(Call &C, const tj_tables *tables, int lcut, const double *d_Wtt, const double *d_Wtp,
                    const double *d_Wpp, int nW, double *d_TT, double *d_TE, double *d_EE, double *d_BB, double *d_EB,
-                   cudaStream_t st)
+                   cudaStream_t st, int nw = 1)
 {
     const Tables &T = tables->T;
     C.T = &T;
+    C.nw = nw;
+    C.nW = nW;
     C.banded = lcut >= 0;
     C.lcut = lcut;
     // an output needs its window (TJ_EINVAL otherwise)
@@ -368,7 +394,7 @@ int coupling_begin(Call &C, const tj_tables *tables, int lcut, const double *d_W
     if (!d_TE && !C.ee && !d_EB) C.mask = M_TT;
     else if (d_TT) C.mask = M_TT | M_TE | M_EE | M_EB;
     else C.mask = M_TE | M_EE | M_EB;
-    C.R = sweep_R(C.mask, C.banded);
+    C.R = sweep_R(C.mask, C.banded, nw);
     C.l3max_eff = C.banded ? lcut : T.l3max;
     C.N = (long long)T.lmax + 1;
     C.ld = C.banded ? (long long)(2 * lcut + 1) : C.N;
@@ -378,7 +404,7 @@ int coupling_begin(Call &C, const tj_tables *tables, int lcut, const double *d_W
     C.ntile_w = (int)((C.N + 31) / 32);
 
     // ---- stream-ordered scratch: 3 prefolded windows + tile prefix
-    const size_t wbytes = sizeof(double) * 3 * (size_t)T.nl_alloc;
+    const size_t wbytes = sizeof(double) * 3 * (size_t)T.nl_alloc * (size_t)nw;
     const size_t tbytes = sizeof(int) * (size_t)(C.nb + 1 + 1);
     const size_t tb_al = (tbytes + 15) & ~(size_t)15;
     TJ_CUDA(cudaMallocAsync((void **)&C.scratch, wbytes + tb_al, st), "coupling/scratch");
@@ -388,12 +414,16 @@ int coupling_begin(Call &C, const tj_tables *tables, int lcut, const double *d_W
     C.tile_start = (int *)(C.scratch + wbytes);
 
     prof_record(0, st);
-    cudaError_t e = launch_prepare(T, d_Wtt, d_Wtp, d_Wpp, nW, C.wtt, C.wtp, C.wpp, C.tile_start, C.R, C.l3max_eff,
-                                   C.banded, st);
+    cudaError_t e = cudaSuccess;
+    for (int w = 0; w < nw && e == cudaSuccess; ++w) {   // window set w: inputs [w][nW], prefolded arrays 3*nl_alloc apart
+        const size_t wi = (size_t)w * (size_t)nW, wo = (size_t)w * 3 * (size_t)T.nl_alloc;
+        e = launch_prepare(T, d_Wtt ? d_Wtt + wi : nullptr, d_Wtp ? d_Wtp + wi : nullptr, d_Wpp ? d_Wpp + wi : nullptr,
+                           nW, C.wtt + wo, C.wtp + wo, C.wpp + wo, C.tile_start, C.R, C.l3max_eff, C.banded, st);
+    }
     prof_record(1, st);
     if (e == cudaSuccess && C.banded) {
         // slots of the band whose l2 falls outside 0..lmax (and everything the sweep does not own) are 0
-        const size_t per = (size_t)C.N * (size_t)C.ld;
+        const size_t per = (size_t)C.N * (size_t)C.ld * (size_t)nw;
         double *outs[5] = {d_TT, d_TE, d_EE, d_BB, d_EB};
         for (int k = 0; k < 5 && e == cudaSuccess; ++k)
             if (outs[k]) e = cudaMemsetAsync(outs[k], 0, sizeof(double) * per, st);
@@ -424,8 +454,10 @@ cudaError_t coupling_sweep(const Call &C, int b0, int b1, cudaStream_t st)
     P.lmax = T.lmax; P.l3max = C.l3max_eff; P.nbands = C.nb; P.lcut = C.banded ? C.lcut : -1; P.ld = C.ld;
     const bool all = (b0 == 0 && b1 == C.nb);
     P.tile_off = all ? 0 : tiles_above(C, b1 - 1);
+    P.wstride = 3 * (long long)T.nl_alloc;
+    P.ostride = C.N * C.ld;
     const int n = all ? C.ntiles : tiles_above(C, b0 - 1) - P.tile_off;
-    return launch_sweep(P, C.mask, n, st);
+    return launch_sweep(P, C.mask, C.nw, n, st);
 }
 
 // scale + mirror of the 32-row tile rows [I0, I1)
@@ -445,7 +477,13 @@ cudaError_t coupling_write(const Call &C, int I0, int I1, cudaStream_t st)
     const int tb = (C.lcut + 31) / 32 + 1;
     W.tile_band = (C.banded && tb < W.ntile - 1) ? tb : W.ntile - 1;
     W.I0 = I0; W.I1 = I1;
-    return launch_writer(W, st);
+    cudaError_t e = cudaSuccess;
+    for (int w = 0; w < C.nw && e == cudaSuccess; ++w) {
+        e = launch_writer(W, st);
+        for (int k = 0; k < W.nmat; ++k) W.M[k] += C.N * C.ld;
+        if (W.bb) W.bb += C.N * C.ld;
+    }
+    return e;
 }
 
 void coupling_end(Call &C, cudaStream_t st)
@@ -455,10 +493,10 @@ void coupling_end(Call &C, cudaStream_t st)
 }
 
 int run_coupling(const tj_tables *tables, int lcut, const double *d_Wtt, const double *d_Wtp, const double *d_Wpp,
-                 int nW, double *d_TT, double *d_TE, double *d_EE, double *d_BB, double *d_EB, cudaStream_t st)
+                 int nW, double *d_TT, double *d_TE, double *d_EE, double *d_BB, double *d_EB, cudaStream_t st, int nw)
 {
     Call C;
-    int rc = coupling_begin(C, tables, lcut, d_Wtt, d_Wtp, d_Wpp, nW, d_TT, d_TE, d_EE, d_BB, d_EB, st);
+    int rc = coupling_begin(C, tables, lcut, d_Wtt, d_Wtp, d_Wpp, nW, d_TT, d_TE, d_EE, d_BB, d_EB, st, nw);
     if (rc != TJ_OK) return rc;
     prof_record(2, st);
     cudaError_t e = coupling_sweep(C, 0, C.nb, st);

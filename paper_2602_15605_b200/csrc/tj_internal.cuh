@@ -23,6 +23,7 @@ constexpr int SWEEP_THREADS = 128;   // columns c per CTA
 constexpr int R_POL = 12;           // pairs per thread, fused TT+TE+EE(+EB) sweep, dense storage
 constexpr int R_POL_BAND = 8;       // same, band-limited (short sweeps)
 constexpr int R_TT = 16;             // pairs per thread, TT-only sweep
+constexpr int R_MULTI2 = 8;         // pairs per thread, 2 window sets per sweep (tj_coupling_multi)
 
 // mask bits of the blocks one sweep computes
 constexpr int M_TT = 1, M_TE = 2, M_EE = 4, M_EB = 8;
@@ -66,6 +67,8 @@ struct SweepParams {
     int lmax, l3max, nbands, lcut;  // lcut < 0: dense storage
     int tile_off;                   // first tile of this launch in the descending-band prefix (row-chunked launches)
     long long ld;                   // row stride of the outputs
+    long long wstride;              // multi-window: doubles between the prefolded arrays of consecutive window sets
+    long long ostride;              // multi-window: doubles between the output matrices of consecutive window sets
 };
 
 struct WriterParams {
@@ -85,8 +88,8 @@ cudaError_t launch_build_tables(const Tables &T, cudaStream_t st);
 cudaError_t launch_prepare(const Tables &T, const double *d_Wtt, const double *d_Wtp, const double *d_Wpp, int nW,
                            double *wtt, double *wtp, double *wpp, int *tile_start, int R, int l3max_eff, bool banded,
                            cudaStream_t st);
-int sweep_R(int mask, bool banded);   // pairs per thread (= rows per band) of the sweep that serves `mask`
-cudaError_t launch_sweep(const SweepParams &P, int mask, int total_tiles, cudaStream_t st);
+int sweep_R(int mask, bool banded, int nw);   // pairs per thread (= rows per band) of the sweep that serves `mask` for nw window sets
+cudaError_t launch_sweep(const SweepParams &P, int mask, int nw, int total_tiles, cudaStream_t st);
 cudaError_t launch_writer(const WriterParams &P, cudaStream_t st);
 cudaError_t launch_fp64_probe(int iters, double *d_sink, int blocks, int threads, cudaStream_t st);
 

@@ -51,6 +51,9 @@
 namespace tj {
 namespace {
 
+#ifndef TJ_TS_DENSE
+#define TJ_TS_DENSE 48   // steps per stage of the dense polarised sweep (a multiple of R_POL, even)
+#endif
 constexpr int NBUF = 2;   // buffers per warp
 constexpr int PAD = 2;    // doubles in front of each slice: the software-pipelined read of "step TS" lands here
 
@@ -85,13 +88,15 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t
 }
 
 // capacities (doubles, all even) of the slices inside one stage buffer
-template <int TS> struct Lay {
+template <int TS, int NW> struct Lay {
     static constexpr int CA = PAD + TS + 2;            // row ring / step factor
     static constexpr int CB = PAD + TS + 32 + 2;       // column ring / h
     static constexpr int CW = PAD + 2 * TS + 32 + 2;   // windows, u3
     static constexpr int OA = 0, OG = OA + CA, OB = OG + CA, OH = OB + CB;
-    static constexpr int OW0 = OH + CB, OW1 = OW0 + CW, OW2 = OW1 + CW, OU = OW2 + CW;
-    static constexpr int BUFD = OU + CW;               // doubles per buffer
+    static constexpr int OU = OH + CB;
+    // NW window sets (multi-window batching): slot w of TT / TP / PP
+    static constexpr int OW0 = OU + CW, OW1 = OW0 + NW * CW, OW2 = OW1 + NW * CW;
+    static constexpr int BUFD = OW2 + NW * CW;         // doubles per buffer
 };
 
 // one slice: n doubles starting at table index i0 (any parity) -> buffer offset off (+PAD)
@@ -108,14 +113,14 @@ __device__ __forceinline__ int slice_bytes(int i0, int n)
     return ((n + (i0 - ie) + 1) & ~1) * 8;
 }
 
-template <int R, int MASK, int TS, int MINB, bool PIPE>
+template <int R, int MASK, int TS, int MINB, bool PIPE, int NW>
 __global__ void __launch_bounds__(SWEEP_THREADS, MINB) sweep_tma_kernel(const __grid_constant__ SweepParams P)
 {
     constexpr bool kTT = (MASK & M_TT) != 0, kTE = (MASK & M_TE) != 0, kEE = (MASK & M_EE) != 0,
                    kEB = (MASK & M_EB) != 0;
     constexpr bool kEven = kTT || kTE || kEE;
     constexpr bool kA2 = kTE || kEE;
-    using L = Lay<TS>;
+    using L = Lay<TS, NW>;
     static_assert(TS % R == 0 && TS % 2 == 0, "stage length: a multiple of R and even");
 
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -167,17 +172,19 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB) sweep_tma_kernel(const __
         if (q < nso) {
             const int t0 = tbo + q * TS, tl = t0 + TS - 1;
             uint32_t bytes = slice_bytes(a - tl, TS) + slice_bytes(t0, TS) + slice_bytes(cw - R + 1 - tl, TS + 31) +
-                             slice_bytes(sw - tl, TS + 31) + 2 * slice_bytes(sw - 2 * tl - 1, 2 * (TS - 1) + 32);
+                             slice_bytes(sw - tl, TS + 31) + (NW + 1) * slice_bytes(sw - 2 * tl - 1, 2 * (TS - 1) + 32);
             mbar_expect_tx(bar, bytes);
             slice(buf, L::OA, P.gA, a - tl, TS, bar);
             slice(buf, L::OG, P.gB, t0, TS, bar);
             slice(buf, L::OB, P.gA, cw - R + 1 - tl, TS + 31, bar);
             slice(buf, L::OH, P.ginv, sw - tl, TS + 31, bar);
-            slice(buf, L::OW2, P.wpp, sw - 2 * tl - 1, 2 * (TS - 1) + 32, bar);
+#pragma unroll
+            for (int w = 0; w < NW; ++w)
+                slice(buf, L::OW2 + w * L::CW, P.wpp + w * P.wstride, sw - 2 * tl - 1, 2 * (TS - 1) + 32, bar);
             slice(buf, L::OU, P.u3, sw - 2 * tl - 1, 2 * (TS - 1) + 32, bar);
         } else {
             const int t0 = tbe + (q - nso) * TS, tl = t0 + TS - 1;
-            const int nwin = (kTT ? 1 : 0) + (kTE ? 1 : 0) + (kEE ? 1 : 0) + (kA2 ? 1 : 0);
+            const int nwin = NW * ((kTT ? 1 : 0) + (kTE ? 1 : 0) + (kEE ? 1 : 0)) + (kA2 ? 1 : 0);
             uint32_t bytes = slice_bytes(a - tl, TS) + slice_bytes(t0, TS) + slice_bytes(cw - R + 1 - tl, TS + 31) +
                              slice_bytes(sw - tl, TS + 31) + nwin * slice_bytes(sw - 2 * tl, 2 * (TS - 1) + 32);
             mbar_expect_tx(bar, bytes);
@@ -185,9 +192,12 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB) sweep_tma_kernel(const __
             slice(buf, L::OG, P.g, t0, TS, bar);
             slice(buf, L::OB, P.g, cw - R + 1 - tl, TS + 31, bar);
             slice(buf, L::OH, P.h, sw - tl, TS + 31, bar);
-            if (kTT) slice(buf, L::OW0, P.wtt, sw - 2 * tl, 2 * (TS - 1) + 32, bar);
-            if (kTE) slice(buf, L::OW1, P.wtp, sw - 2 * tl, 2 * (TS - 1) + 32, bar);
-            if (kEE) slice(buf, L::OW2, P.wpp, sw - 2 * tl, 2 * (TS - 1) + 32, bar);
+#pragma unroll
+            for (int w = 0; w < NW; ++w) {
+                if (kTT) slice(buf, L::OW0 + w * L::CW, P.wtt + w * P.wstride, sw - 2 * tl, 2 * (TS - 1) + 32, bar);
+                if (kTE) slice(buf, L::OW1 + w * L::CW, P.wtp + w * P.wstride, sw - 2 * tl, 2 * (TS - 1) + 32, bar);
+                if (kEE) slice(buf, L::OW2 + w * L::CW, P.wpp + w * P.wstride, sw - 2 * tl, 2 * (TS - 1) + 32, bar);
+            }
             if (kA2) slice(buf, L::OU, P.u3, sw - 2 * tl, 2 * (TS - 1) + 32, bar);
         }
     };
@@ -213,9 +223,11 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB) sweep_tma_kernel(const __
 
     // =========================== odd-J branch: EB ===========================
     if (kEB) {
-        double acc[R];
+        double acc[NW][R];
 #pragma unroll
-        for (int i = 0; i < R; ++i) acc[i] = 0.0;
+        for (int w = 0; w < NW; ++w)
+#pragma unroll
+            for (int i = 0; i < R; ++i) acc[w][i] = 0.0;
         if (nso > 0) {
             double wa[R], wb[R];
             {   // ring start-up straight from global memory (once per warp)
@@ -239,7 +251,10 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB) sweep_tma_kernel(const __
                 const double *sb = wbuf + b * L::BUFD;
                 const double *pa = sb + oa, *pg = sb + og, *pb = sb + ob, *ph = sb + oh;
                 const double *pw = sb + L::OW2 + ow, *pu = sb + L::OU + ow;
-                double xa = pa[0], xb = pb[0], xh = ph[0], xg = pg[0], xw = pw[0], xu = pu[0];
+                double xa = pa[0], xb = pb[0], xh = ph[0], xg = pg[0], xu = pu[0];
+                double xw[NW];
+#pragma unroll
+                for (int w = 0; w < NW; ++w) xw[w] = pw[w * L::CW];
 #pragma unroll 1
                 for (int blk = 0; blk < TS / R; ++blk) {
 #pragma unroll
@@ -247,10 +262,14 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB) sweep_tma_kernel(const __
                         wa[(R - u) % R] = xa;
                         wb[(R + 1 - u) % R] = xb;
                         const double hg = __dmul_rn(xh, xg);
-                        const double q3 = __dmul_rn(xw, hg);
+                        double q3[NW];
+#pragma unroll
+                        for (int w = 0; w < NW; ++w) q3[w] = __dmul_rn(xw[w], hg);
                         const double c3 = xu;
                         xa = pa[-(u + 1)]; xb = pb[-(u + 1)]; xh = ph[-(u + 1)]; xg = pg[u + 1];
-                        xw = pw[-2 * (u + 1)]; xu = pu[-2 * (u + 1)];
+#pragma unroll
+                        for (int w = 0; w < NW; ++w) xw[w] = pw[w * L::CW - 2 * (u + 1)];
+                        xu = pu[-2 * (u + 1)];
                         double r[R], e[R];
 #pragma unroll
                         for (int i = 0; i < R; ++i) r[i] = __dmul_rn(wa[(i - u + R) % R], wb[(2 * R - i - u) % R]);
@@ -261,7 +280,9 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB) sweep_tma_kernel(const __
 #pragma unroll
                         for (int i = 0; i < R; ++i) r[i] = __dmul_rn(r[i], e[i]);
 #pragma unroll
-                        for (int i = 0; i < R; ++i) acc[i] = __fma_rn(r[i], q3, acc[i]);
+                        for (int w = 0; w < NW; ++w)
+#pragma unroll
+                            for (int i = 0; i < R; ++i) acc[w][i] = __fma_rn(r[i], q3[w], acc[w][i]);
                     }
                     pa -= R; pb -= R; ph -= R; pg += R; pw -= 2 * R; pu -= 2 * R;
                 }
@@ -276,20 +297,26 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB) sweep_tma_kernel(const __
             if (l2 >= l1 && l2 <= P.lmax && (P.lcut < 0 || l2 - l1 <= P.lcut)) {
                 const double sd = P.isd[l1] * P.isd[l2];
                 const long long col = P.lcut < 0 ? (long long)l2 : (long long)(l2 - l1 + P.lcut);
-                if (P.EB) P.EB[(long long)l1 * P.ld + col] = acc[i] * (0.25 * sd * sd);
+                if (P.EB) {
+#pragma unroll
+                    for (int w = 0; w < NW; ++w)
+                        P.EB[w * P.ostride + (long long)l1 * P.ld + col] = acc[w][i] * (0.25 * sd * sd);
+                }
             }
         }
     }
 
     // =========================== even-J branch: TT, TE, EE ===========================
     if (kEven) {
-        double att[kTT ? R : 1], ate[kTE ? R : 1], aee[kEE ? R : 1];
+        double att[NW][kTT ? R : 1], ate[NW][kTE ? R : 1], aee[NW][kEE ? R : 1];
 #pragma unroll
-        for (int i = 0; i < R; ++i) {
-            if (kTT) att[i] = 0.0;
-            if (kTE) ate[i] = 0.0;
-            if (kEE) aee[i] = 0.0;
-        }
+        for (int w = 0; w < NW; ++w)
+#pragma unroll
+            for (int i = 0; i < R; ++i) {
+                if (kTT) att[w][i] = 0.0;
+                if (kTE) ate[w][i] = 0.0;
+                if (kEE) aee[w][i] = 0.0;
+            }
         if (kA2) {
 #pragma unroll
             for (int i = 0; i < R; ++i) c12[i] += 1.0;   // even branch: d1 = d+1 = u3 - (u1+u2-1)
@@ -305,7 +332,9 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB) sweep_tma_kernel(const __
                 for (int i = 0; i < R - 1; ++i) wb[(R - i) % R] = __ldg(pb + (R - 1 - i));
             }
             // PIPE: products of step t are accumulated at the start of step t+1 (see the loop body)
-            double rA[kTE ? R : 1], rAA[kEE ? R : 1], p1 = 0.0, p2 = 0.0;
+            double rA[kTE ? R : 1], rAA[kEE ? R : 1], p1[NW], p2[NW];
+#pragma unroll
+            for (int w = 0; w < NW; ++w) { p1[w] = 0.0; p2[w] = 0.0; }
 #pragma unroll
             for (int i = 0; i < R; ++i) { if (kTE) rA[i] = 0.0; if (kEE) rAA[i] = 0.0; }
             const int tl0 = tbe + TS - 1;
@@ -322,7 +351,13 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB) sweep_tma_kernel(const __
                 const double *pwtt = sb + L::OW0 + ow, *pwtp = sb + L::OW1 + ow, *pwpp = sb + L::OW2 + ow;
                 const double *pu = sb + L::OU + ow;
                 double xa = pa[0], xb = pb[0], xh = ph[0], xg = pg[0];
-                double xtt = kTT ? pwtt[0] : 0.0, xtp = kTE ? pwtp[0] : 0.0, xpp = kEE ? pwpp[0] : 0.0;
+                double xtt[NW], xtp[NW], xpp[NW];
+#pragma unroll
+                for (int w = 0; w < NW; ++w) {
+                    xtt[w] = kTT ? pwtt[w * L::CW] : 0.0;
+                    xtp[w] = kTE ? pwtp[w * L::CW] : 0.0;
+                    xpp[w] = kEE ? pwpp[w * L::CW] : 0.0;
+                }
                 double xu = kA2 ? pu[0] : 0.0;
 #pragma unroll 1
                 for (int blk = 0; blk < TS / R; ++blk) {
@@ -331,35 +366,46 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB) sweep_tma_kernel(const __
                         wa[(R - u) % R] = xa;
                         wb[(R + 1 - u) % R] = xb;
                         const double hg = __dmul_rn(xh, xg);
-                        double q0 = 0.0, q1 = 0.0, q2 = 0.0;
-                        if (kTT) q0 = __dmul_rn(xtt, hg);
-                        if (kTE) q1 = __dmul_rn(xtp, hg);
-                        if (kEE) q2 = __dmul_rn(xpp, hg);
+                        double q0[NW], q1[NW], q2[NW];
+#pragma unroll
+                        for (int w = 0; w < NW; ++w) {
+                            q0[w] = kTT ? __dmul_rn(xtt[w], hg) : 0.0;
+                            q1[w] = kTE ? __dmul_rn(xtp[w], hg) : 0.0;
+                            q2[w] = kEE ? __dmul_rn(xpp[w], hg) : 0.0;
+                        }
                         const double c3 = xu;
                         xa = pa[-(u + 1)]; xb = pb[-(u + 1)]; xh = ph[-(u + 1)]; xg = pg[u + 1];
-                        if (kTT) xtt = pwtt[-2 * (u + 1)];
-                        if (kTE) xtp = pwtp[-2 * (u + 1)];
-                        if (kEE) xpp = pwpp[-2 * (u + 1)];
+#pragma unroll
+                        for (int w = 0; w < NW; ++w) {
+                            if (kTT) xtt[w] = pwtt[w * L::CW - 2 * (u + 1)];
+                            if (kTE) xtp[w] = pwtp[w * L::CW - 2 * (u + 1)];
+                            if (kEE) xpp[w] = pwpp[w * L::CW - 2 * (u + 1)];
+                        }
                         if (kA2) xu = pu[-2 * (u + 1)];
                         if (PIPE) {
                         // accumulate the PREVIOUS step's products first (their inputs are long ready, so the
                         // 8 FMAs of one window issue back to back and share q through the operand reuse cache)
-                        if (kTE) {
 #pragma unroll
-                            for (int i = 0; i < R; ++i) ate[i] = __fma_rn(rA[i], p1, ate[i]);
-                        }
-                        if (kEE) {
+                        for (int w = 0; w < NW; ++w) {
+                            if (kTE) {
 #pragma unroll
-                            for (int i = 0; i < R; ++i) aee[i] = __fma_rn(rAA[i], p2, aee[i]);
+                                for (int i = 0; i < R; ++i) ate[w][i] = __fma_rn(rA[i], p1[w], ate[w][i]);
+                            }
+                            if (kEE) {
+#pragma unroll
+                                for (int i = 0; i < R; ++i) aee[w][i] = __fma_rn(rAA[i], p2[w], aee[w][i]);
+                            }
+                            p1[w] = q1[w]; p2[w] = q2[w];
                         }
-                        p1 = q1; p2 = q2;
                         }
                         double r[R], A2[kA2 ? R : 1];
 #pragma unroll
                         for (int i = 0; i < R; ++i) r[i] = __dmul_rn(wa[(i - u + R) % R], wb[(2 * R - i - u) % R]);
                         if (kTT) {
 #pragma unroll
-                            for (int i = 0; i < R; ++i) att[i] = __fma_rn(r[i], q0, att[i]);
+                            for (int w = 0; w < NW; ++w)
+#pragma unroll
+                                for (int i = 0; i < R; ++i) att[w][i] = __fma_rn(r[i], q0[w], att[w][i]);
                         }
                         if (kA2) {
 #pragma unroll
@@ -374,13 +420,16 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB) sweep_tma_kernel(const __
                             }
                         }
                         if (!PIPE) {
-                        if (kTE) {
 #pragma unroll
-                            for (int i = 0; i < R; ++i) ate[i] = __fma_rn(rA[i], q1, ate[i]);
-                        }
-                        if (kEE) {
+                        for (int w = 0; w < NW; ++w) {
+                            if (kTE) {
 #pragma unroll
-                            for (int i = 0; i < R; ++i) aee[i] = __fma_rn(rAA[i], q2, aee[i]);
+                                for (int i = 0; i < R; ++i) ate[w][i] = __fma_rn(rA[i], q1[w], ate[w][i]);
+                            }
+                            if (kEE) {
+#pragma unroll
+                                for (int i = 0; i < R; ++i) aee[w][i] = __fma_rn(rAA[i], q2[w], aee[w][i]);
+                            }
                         }
                         }
                     }
@@ -393,8 +442,11 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB) sweep_tma_kernel(const __
             if (PIPE) {
 #pragma unroll
             for (int i = 0; i < R; ++i) {   // the last step's products
-                if (kTE) ate[i] = __fma_rn(rA[i], p1, ate[i]);
-                if (kEE) aee[i] = __fma_rn(rAA[i], p2, aee[i]);
+#pragma unroll
+                for (int w = 0; w < NW; ++w) {
+                    if (kTE) ate[w][i] = __fma_rn(rA[i], p1[w], ate[w][i]);
+                    if (kEE) aee[w][i] = __fma_rn(rAA[i], p2[w], aee[w][i]);
+                }
             }
             }
         }
@@ -405,59 +457,67 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB) sweep_tma_kernel(const __
             if (l2 >= l1 && l2 <= P.lmax && (P.lcut < 0 || l2 - l1 <= P.lcut)) {
                 const long long col = P.lcut < 0 ? (long long)l2 : (long long)(l2 - l1 + P.lcut);
                 const long long idx = (long long)l1 * P.ld + col;
-                if (kTT && P.TT) P.TT[idx] = att[i];
-                if (kA2) {
-                    const double sd = P.isd[l1] * P.isd[l2];
-                    if (kTE && P.TE) P.TE[idx] = ate[i] * (0.5 * sd);
-                    if (kEE && P.EE) P.EE[idx] = aee[i] * (0.25 * sd * sd);
+                const double sd = kA2 ? P.isd[l1] * P.isd[l2] : 0.0;
+#pragma unroll
+                for (int w = 0; w < NW; ++w) {
+                    const long long iw = idx + w * P.ostride;
+                    if (kTT && P.TT) P.TT[iw] = att[w][i];
+                    if (kTE && P.TE) P.TE[iw] = ate[w][i] * (0.5 * sd);
+                    if (kEE && P.EE) P.EE[iw] = aee[w][i] * (0.25 * sd * sd);
                 }
             }
         }
     }
 }
 
-template <int R, int MASK, int TS, int MINB, bool PIPE>
+template <int R, int MASK, int TS, int MINB, bool PIPE, int NW = 1>
 cudaError_t launch_one(const SweepParams &P, int total_tiles, cudaStream_t st)
 {
     if (total_tiles <= 0) return cudaSuccess;
     constexpr int NWARP = SWEEP_THREADS / 32;
-    constexpr size_t smem = (size_t)NWARP * NBUF * Lay<TS>::BUFD * 8 + (size_t)NWARP * NBUF * 8;
+    constexpr size_t smem = (size_t)NWARP * NBUF * Lay<TS, NW>::BUFD * 8 + (size_t)NWARP * NBUF * 8;
     static bool attr_set = false;   // per instantiation
     if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(sweep_tma_kernel<R, MASK, TS, MINB, PIPE>,
+        cudaError_t e = cudaFuncSetAttribute(sweep_tma_kernel<R, MASK, TS, MINB, PIPE, NW>,
                                              cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         attr_set = true;
     }
-    sweep_tma_kernel<R, MASK, TS, MINB, PIPE><<<total_tiles, SWEEP_THREADS, smem, st>>>(P);
+    sweep_tma_kernel<R, MASK, TS, MINB, PIPE, NW><<<total_tiles, SWEEP_THREADS, smem, st>>>(P);
     return cudaGetLastError();
 }
 
 }  // namespace
 
 // Geometry per request: dense sweeps are long (up to lmax steps per pair), so the per-step
-// overhead (prefactors, table reads) is spread over R = 12 pairs at 2 CTAs/SM with stages of 48 steps;
+// overhead (prefactors, table reads) is spread over R = 12 pairs at 2 CTAs/SM with stages of TJ_TS_DENSE steps;
 // band-limited sweeps have <= lcut/2+1 steps per pair, so they keep R = 8 and short stages of 32 steps.
-int sweep_R(int mask, bool banded)
+// Multi-window batching (nw window sets in one sweep): the geometric part of a term (r, A2, rA, rAA) is
+// computed once and each window set adds 3 FMAs (1 in the odd branch); the accumulators of nw sets take the
+// registers that R = 12 pairs use otherwise, hence R = 8 for nw = 2 (the only batched instantiation).
+int sweep_R(int mask, bool banded, int nw)
 {
+    if (nw == 2) return R_MULTI2;
     if (mask == M_TT) return R_TT;
     return banded ? R_POL_BAND : R_POL;
 }
 
-cudaError_t launch_sweep(const SweepParams &P, int mask, int total_tiles, cudaStream_t st)
+cudaError_t launch_sweep(const SweepParams &P, int mask, int nw, int total_tiles, cudaStream_t st)
 {
     constexpr int POL = M_TE | M_EE | M_EB, ALL = M_TT | POL;
     const bool banded = P.lcut >= 0;
+    if (nw == 2 && !banded && mask == ALL) return launch_one<R_MULTI2, ALL, 48, 2, true, 2>(P, total_tiles, st);
+    if (nw != 1) return cudaErrorInvalidValue;
     switch (mask) {
         case M_TT:
             return banded ? launch_one<R_TT, M_TT, 32, 3, false>(P, total_tiles, st)
                           : launch_one<R_TT, M_TT, 48, 3, false>(P, total_tiles, st);
         case POL:
             return banded ? launch_one<R_POL_BAND, POL, 32, 3, false>(P, total_tiles, st)
-                          : launch_one<R_POL, POL, 48, 2, true>(P, total_tiles, st);
+                          : launch_one<R_POL, POL, TJ_TS_DENSE, 2, true>(P, total_tiles, st);
         case ALL:
             return banded ? launch_one<R_POL_BAND, ALL, 32, 3, false>(P, total_tiles, st)
-                          : launch_one<R_POL, ALL, 48, 2, true>(P, total_tiles, st);
+                          : launch_one<R_POL, ALL, TJ_TS_DENSE, 2, true>(P, total_tiles, st);
         default: return cudaErrorInvalidValue;
     }
 }

@@ -380,3 +380,46 @@ def test_cfg4_band_full_size_sampled():
     # rows 0 and lmax: out-of-range slots zero
     assert torch.all(out["TT"][0, :lcut] == 0) and torch.all(out["TT"][-1, lcut + 1:] == 0)
     T.close()
+
+
+# ---------------------------------------------------------------- multi-window batching
+def _window_sets(lmax, nwin, seed):
+    """nwin independent window sets of the config-1 recipe (different seeds)."""
+    sets = [windows.pol_windows(lmax, (0.7, 30.0, 2.5), (0.5, 50.0, 3.0), 0.05, seed + k) for k in range(nwin)]
+    return [np.stack([s[j] for s in sets]) for j in range(3)]
+
+
+def test_multi_window_against_oracle():
+    """3 window sets in one call (one batched pair + one single sweep), each against the oracle."""
+    import torch
+    lmax, nwin = 150, 3
+    Wtt, Wtp, Wpp = _window_sets(lmax, nwin, 100)
+    T = binding.build_tables(lmax)
+    out = binding.coupling_multi(T, _t(Wtt), _t(Wtp), _t(Wpp))
+    torch.cuda.synchronize()
+    for w in range(nwin):
+        ref = oracle.coupling_full(lmax, 2 * lmax, Wtt[w], Wtp[w], Wpp[w])
+        for k in BLOCKS:
+            assert_parity(out[k][w].cpu().numpy(), ref[k], "multi set %d %s" % (w, k))
+    T.close()
+
+
+def test_multi_window_equals_single_calls_bitwise():
+    """The batched sweep forms every entry with the same operations in the same order as tj_coupling_pol."""
+    import torch
+    lmax, nwin = 777, 5
+    Wtt, Wtp, Wpp = _window_sets(lmax, nwin, 200)
+    T = binding.build_tables(lmax)
+    out = binding.coupling_multi(T, _t(Wtt), _t(Wtp), _t(Wpp))
+    torch.cuda.synchronize()
+    for w in range(nwin):
+        one = binding.coupling_pol(T, _t(Wtt[w]), _t(Wtp[w]), _t(Wpp[w]))
+        torch.cuda.synchronize()
+        for k in BLOCKS:
+            assert torch.equal(out[k][w], one[k]), (w, k)
+    # partial requests take the one-set-per-sweep route
+    part = binding.coupling_multi(T, None, None, _t(Wpp), want=("EE", "EB"))
+    torch.cuda.synchronize()
+    for w in range(nwin):
+        assert torch.equal(part["EE"][w], out["EE"][w]) and torch.equal(part["EB"][w], out["EB"][w])
+    T.close()
