@@ -51,9 +51,11 @@
 namespace tj {
 namespace {
 
-#ifndef TJ_TS_DENSE
-#define TJ_TS_DENSE 48   // steps per stage of the dense polarised sweep (a multiple of R_POL, even)
-#endif
+// steps per stage of the dense polarised sweep (a multiple of R_POL, even): long stages amortise the stage
+// turn-over (measured at lmax = 10^4: TS = 24 148.8 ms, 48 143.4 ms, 96 141.7 ms) but round every warp's walk
+// up to whole stages, so short sweeps keep the short stage
+constexpr int TS_DENSE_LONG = 96, TS_DENSE_SHORT = 48;
+constexpr int LMAX_LONG_STAGES = 4096;
 constexpr int NBUF = 2;   // buffers per warp
 constexpr int PAD = 2;    // doubles in front of each slice: the software-pipelined read of "step TS" lands here
 
@@ -490,7 +492,7 @@ cudaError_t launch_one(const SweepParams &P, int total_tiles, cudaStream_t st)
 }  // namespace
 
 // Geometry per request: dense sweeps are long (up to lmax steps per pair), so the per-step
-// overhead (prefactors, table reads) is spread over R = 12 pairs at 2 CTAs/SM with stages of TJ_TS_DENSE steps;
+// overhead (prefactors, table reads) is spread over R = 12 pairs at 2 CTAs/SM with stages of 96 (48) steps;
 // band-limited sweeps have <= lcut/2+1 steps per pair, so they keep R = 8 and short stages of 32 steps.
 // Multi-window batching (nw window sets in one sweep): the geometric part of a term (r, A2, rA, rAA) is
 // computed once and each window set adds 3 FMAs (1 in the odd branch); the accumulators of nw sets take the
@@ -514,10 +516,12 @@ cudaError_t launch_sweep(const SweepParams &P, int mask, int nw, int total_tiles
                           : launch_one<R_TT, M_TT, 48, 3, false>(P, total_tiles, st);
         case POL:
             return banded ? launch_one<R_POL_BAND, POL, 32, 3, false>(P, total_tiles, st)
-                          : launch_one<R_POL, POL, TJ_TS_DENSE, 2, true>(P, total_tiles, st);
+                          : (P.lmax >= LMAX_LONG_STAGES ? launch_one<R_POL, POL, TS_DENSE_LONG, 2, true>(P, total_tiles, st)
+                                                        : launch_one<R_POL, POL, TS_DENSE_SHORT, 2, true>(P, total_tiles, st));
         case ALL:
             return banded ? launch_one<R_POL_BAND, ALL, 32, 3, false>(P, total_tiles, st)
-                          : launch_one<R_POL, ALL, TJ_TS_DENSE, 2, true>(P, total_tiles, st);
+                          : (P.lmax >= LMAX_LONG_STAGES ? launch_one<R_POL, ALL, TS_DENSE_LONG, 2, true>(P, total_tiles, st)
+                                                        : launch_one<R_POL, ALL, TS_DENSE_SHORT, 2, true>(P, total_tiles, st));
         default: return cudaErrorInvalidValue;
     }
 }
