@@ -19,6 +19,8 @@ from .coupling import (  # noqa: F401
     coupling_rows,
     coupling_full,
     coupling_band,
+    spin1_pairs,
+    spin1_full,
     num_threads,
     set_num_threads,
 )

@@ -44,6 +44,8 @@ def lib() -> ctypes.CDLL:
         L.oracle_l3_range.restype = ctypes.c_int
         L.oracle_coupling_pairs.argtypes = [ctypes.c_int, dp, dp, dp, ctypes.c_long, ip, ip, dp, dp, dp, dp]
         L.oracle_coupling_pairs.restype = ctypes.c_int
+        L.oracle_coupling_spin1_pairs.argtypes = [ctypes.c_int, dp, dp, ctypes.c_long, ip, ip, dp, dp, dp]
+        L.oracle_coupling_spin1_pairs.restype = ctypes.c_int
         L.oracle_num_threads.restype = ctypes.c_int
         L.oracle_set_num_threads.argtypes = [ctypes.c_int]
         _LIB = L
@@ -156,3 +158,32 @@ def coupling_band(lmax, lcut, Wtt, Wtp, Wpp, rows=None):
         b[ok] = v
         out[k] = b.reshape(rows.size, width)
     return out
+
+
+def spin1_pairs(l3max, W01, W11, l1s, l2s):
+    """Spin-1 blocks K^{01}, K^{11+}, K^{11-} (sg_oracle.c: oracle_coupling_spin1_pairs) for the given pairs."""
+    W01, W11 = _win(W01, l3max), _win(W11, l3max)
+    l1s = np.ascontiguousarray(l1s, dtype=np.int32)
+    l2s = np.ascontiguousarray(l2s, dtype=np.int32)
+    n = l1s.size
+    out = {}
+    if W01 is not None:
+        out["K01"] = np.zeros(n)
+    if W11 is not None:
+        out["K11p"] = np.zeros(n)
+        out["K11m"] = np.zeros(n)
+    ip = ctypes.POINTER(ctypes.c_int)
+    rc = lib().oracle_coupling_spin1_pairs(int(l3max), _dptr(W01), _dptr(W11), n, l1s.ctypes.data_as(ip),
+                                           l2s.ctypes.data_as(ip), _dptr(out.get("K01")), _dptr(out.get("K11p")),
+                                           _dptr(out.get("K11m")))
+    if rc != 0:
+        raise RuntimeError("oracle_coupling_spin1_pairs failed: %d" % rc)
+    return out
+
+
+def spin1_full(lmax, l3max, W01, W11):
+    """All (lmax+1)^2 entries of the spin-1 blocks."""
+    N = lmax + 1
+    l1s = np.repeat(np.arange(N, dtype=np.int32), N)
+    l2s = np.tile(np.arange(N, dtype=np.int32), N)
+    return {k: v.reshape(N, N) for k, v in spin1_pairs(l3max, W01, W11, l1s, l2s).items()}

@@ -22,7 +22,8 @@
  *
  * Pins (tests/test_oracle_*.py): exact Racah rationals for all l <= 30 and a few
  * high-l symbols, orthogonality, parity zeros, full-sky identity, flat-window
- * closed form.  No function in this file is "parity unpinned".
+ * closed form; the spin-1 sums: exact Racah (-1,1,0) symbols, full-sky and flat-window closed forms,
+ * brute-force exact-rational sums.  No function in this file is "parity unpinned".
  */
 #include <math.h>
 #include <stdlib.h>
@@ -246,6 +247,69 @@ int oracle_coupling_pairs(int l3max, const double *Wtt, const double *Wtp, const
         if (EE) EE[q] = pref * see;
         if (EB) EB[q] = pref * seb;
         free(f0); free(f2);
+    }
+    return status;
+}
+
+/*
+ * Spin-1 analogue of Eqs. A1-A4 for a list of (l1,l2) pairs: the same sums with the (0,-1,1) symbol the paper
+ * lists for lensing / aberration weights (symbol formulas PAPER.md:362-392 Eqs. B1-B6) in
+ * place of the spin-2 one.  The paper defines no weights for these, so the blocks are defined here
+ * (reading 19) as
+ *   K^{01}_{l1 l2}  = (2 l2+1)/(4 pi) sum_{l3, J even} (2 l3+1) W^{01}_{l3} (l1 l2 l3;000) (l1 l2 l3;-1 1 0)
+ *   K^{11+}_{l1 l2} = (2 l2+1)/(4 pi) sum_{l3, J even} (2 l3+1) W^{11}_{l3} (l1 l2 l3;-1 1 0)^2
+ *   K^{11-}_{l1 l2} = (2 l2+1)/(4 pi) sum_{l3, J odd } (2 l3+1) W^{11}_{l3} (l1 l2 l3;-1 1 0)^2
+ * with (l1 l2 l3;-1 1 0) = (l3 l1 l2;0 -1 1) (Eq. 7) from the same Schulten-Gordon recursion.
+ * Entries with min(l1,l2) < 1 are 0.  Outputs may be NULL.
+ */
+int oracle_coupling_spin1_pairs(int l3max, const double *W01, const double *W11, long npairs, const int *l1s,
+                                const int *l2s, double *K01, double *K11p, double *K11m)
+{
+    if (l3max < 0 || npairs < 0) return ORACLE_EINVAL;
+    if ((K01 && !W01) || ((K11p || K11m) && !W11)) return ORACLE_EINVAL;
+    int status = ORACLE_OK;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (long q = 0; q < npairs; ++q) {
+        int l1 = l1s[q], l2 = l2s[q];
+        if (l1 < 0 || l2 < 0) {
+#pragma omp atomic write
+            status = ORACLE_EINVAL;
+            continue;
+        }
+        int n = l1 + l2 - abs(l1 - l2) + 1;
+        double *f0 = (double *)malloc(sizeof(double) * (size_t)n);
+        double *f1 = (double *)malloc(sizeof(double) * (size_t)n);
+        if (!f0 || !f1) {
+            free(f0); free(f1);
+#pragma omp atomic write
+            status = ORACLE_ENOMEM;
+            continue;
+        }
+        int jmin, jmax;
+        oracle_3j_family(l1, l2, 0, 0, f0, &jmin, &jmax);
+        if (l1 >= 1 && l2 >= 1) {
+            int jmin1, jmax1;
+            oracle_3j_family(l1, l2, -1, 1, f1, &jmin1, &jmax1);   /* m1 = 0: same j range as f0 */
+        } else {
+            for (int k = 0; k < n; ++k) f1[k] = 0.0;
+        }
+        double s01 = 0.0, s11p = 0.0, s11m = 0.0;
+        int hi = jmax < l3max ? jmax : l3max;
+        for (int l3 = jmin; l3 <= hi; ++l3) {
+            int k = l3 - jmin;
+            double w = 2.0 * l3 + 1.0;
+            if (((l1 + l2 + l3) & 1) == 0) {
+                if (W01) s01 += w * W01[l3] * f0[k] * f1[k];
+                if (W11) s11p += w * W11[l3] * f1[k] * f1[k];
+            } else {
+                if (W11) s11m += w * W11[l3] * f1[k] * f1[k];
+            }
+        }
+        double pref = (2.0 * l2 + 1.0) / (4.0 * PI);
+        if (K01) K01[q] = pref * s01;
+        if (K11p) K11p[q] = pref * s11p;
+        if (K11m) K11m[q] = pref * s11m;
+        free(f0); free(f1);
     }
     return status;
 }

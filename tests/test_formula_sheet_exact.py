@@ -134,3 +134,26 @@ def test_whole_sums_random_rational_windows():
                 assert ee / (4 * D) == ree
                 assert eb / (4 * D) == reb
                 assert te / 2 == rte_times_sqrtD
+
+
+def test_spin1_one_product_forms():
+    """Spin-1 analogues (PAPER.md:362-392 Eqs. B1-B6, B10 carried to one table product):
+       even J: (l1 l2 l3;-1 1 0) = X d / (2 sqrt(u1 u2)),  d = u3 - u1 - u2   (square and sign)
+       odd  J: (l1 l2 l3;-1 1 0)^2 = ginv[s-t] gB[t] gA[l1-t] gA[l2-t] / (4 u1 u2)."""
+    for l1 in range(1, LMAX + 1):
+        for l2 in range(1, LMAX + 1):
+            s = l1 + l2
+            for t in range(0, min(l1, l2) + 1):
+                l3 = s - 2 * t
+                d = u(l3) - u(l1) - u(l2)
+                x2, sx = threej_sq_sign(l1, l2, l3, 0, 0, 0)
+                y2, sy = threej_sq_sign(l1, l2, l3, -1, 1, 0)
+                assert y2 == x2 * Fraction(d * d, 4 * u(l1) * u(l2)), (l1, l2, l3)
+                assert sx * sy == (d > 0) - (d < 0), (l1, l2, l3)
+            for t in range(0, min(l1, l2)):
+                l3 = s - 2 * t - 1
+                gB = (2 * t + 1) * g(t)
+                gA1 = 2 * (l1 - t) * g(l1 - t)
+                gA2 = 2 * (l2 - t) * g(l2 - t)
+                y2, _ = threej_sq_sign(l1, l2, l3, -1, 1, 0)
+                assert y2 == gB * gA1 * gA2 / g(s - t) / (4 * u(l1) * u(l2)), (l1, l2, l3)

@@ -57,7 +57,7 @@ def test_oracle_matches_golden():
         assert abs(v - exact) <= 4e-16 * max(1.0, abs(exact)) + 1e-17, (j1, j2, j3, v, exact)
 
 
-@pytest.mark.parametrize("m2,m3", [(0, 0), (-2, 2)])
+@pytest.mark.parametrize("m2,m3", [(0, 0), (-2, 2), (-1, 1)])
 def test_oracle_vs_racah_all_l_le_30(m2, m3):
     """Every (l1,l2,l3) with l1,l2 <= 30: value within 4e-15 of the family scale of the exact
     rational's root, square within 1e-13 relative wherever the symbol is not near a node, sign exact."""
