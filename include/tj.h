@@ -56,7 +56,7 @@ int tj_tables_info(const tj_tables *tables, int *lmax, int *l3max, int *pmax);
 /*
  * tj_tables_copy -- copy one table to HOST memory (synchronous; for tests of the table kernel).
  *   which: 0 g, 1 ginv, 2 h, 3 gA, 4 gB  (count <= pmax+1 entries, p = 0..count-1);
- *          5 u_l, 6 1/sqrt(D_l)          (count <= lmax+1 entries).
+ *          5 u_l, 6 1/sqrt(D_l), 7 1/sqrt(u_l)   (count <= lmax+1 entries).
  */
 int tj_tables_copy(const tj_tables *tables, int which, double *h_dst, int count);
 
@@ -103,6 +103,23 @@ int tj_coupling_band(const tj_tables *tables, int lcut,
 int tj_coupling_multi(const tj_tables *tables, int nwin,
                       const double *d_Wtt, const double *d_Wtp, const double *d_Wpp, int nW,
                       double *d_TT, double *d_TE, double *d_EE, double *d_BB, double *d_EB,
+                      void *cuda_stream);
+
+/*
+ * tj_coupling_spin1 -- the spin-1 analogue of tj_coupling_pol: the same fused sweep with
+ * the (0,-1,1) symbol the paper lists for lensing / aberration weights (Eqs. B1-B6, B10 at
+ * PAPER.md:362-392, :414-417) in place of the spin-2 one.  The paper defines no weights for it; the blocks are
+ * defined here by analogy with Eqs. A1-A4 (reading 19):
+ *   K00  = TT of tj_coupling_pol                                                 (window W00)
+ *   K01  = (2l2+1)/(4pi) sum_{l3, J even} (2l3+1) W01_l3 (l1 l2 l3;000)(l1 l2 l3;-1 1 0)
+ *   K11p = (2l2+1)/(4pi) sum_{l3, J even} (2l3+1) W11_l3 (l1 l2 l3;-1 1 0)^2
+ *   K11m = the same sum over odd J.
+ * Rows/columns l < 1 of K01, K11p, K11m are exactly 0.0.  NULL rules as tj_coupling_pol (K00 needs W00,
+ * K01 needs W01, K11p/K11m need W11).  Windows: nW = l3max+1 entries; outputs (lmax+1)^2 doubles.
+ */
+int tj_coupling_spin1(const tj_tables *tables,
+                      const double *d_W00, const double *d_W01, const double *d_W11, int nW,
+                      double *d_K00, double *d_K01, double *d_K11p, double *d_K11m,
                       void *cuda_stream);
 
 /*

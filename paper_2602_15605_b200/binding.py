@@ -18,7 +18,7 @@ TJ_OK, TJ_EINVAL, TJ_ENOMEM, TJ_ECUDA = 0, -1, -2, -3
 # every symbol include/tj.h declares (tests/test_abi.py checks the header against this and the .so)
 SYMBOLS = (
     "tj_build_tables", "tj_free_tables", "tj_tables_info", "tj_tables_copy",
-    "tj_coupling_tt", "tj_coupling_pol", "tj_coupling_band", "tj_coupling_multi", "tj_coupling_host",
+    "tj_coupling_tt", "tj_coupling_pol", "tj_coupling_band", "tj_coupling_multi", "tj_coupling_spin1", "tj_coupling_host",
     "tj_l3_range", "tj_sweep_counts", "tj_fp64_probe", "tj_profile_enable", "tj_profile_get",
     "tj_launches_per_call", "tj_strerror",
 )
@@ -53,6 +53,7 @@ def load_library() -> ctypes.CDLL:
     L.tj_coupling_pol.argtypes = [vp, vp, vp, vp, ci, vp, vp, vp, vp, vp, vp]
     L.tj_coupling_band.argtypes = [vp, ci, vp, vp, vp, vp, vp, vp, vp, vp, vp]
     L.tj_coupling_multi.argtypes = [vp, ci, vp, vp, vp, ci, vp, vp, vp, vp, vp, vp]
+    L.tj_coupling_spin1.argtypes = [vp, vp, vp, vp, ci, vp, vp, vp, vp, vp]
     L.tj_coupling_host.argtypes = [vp, ci, ci, vp, vp, vp, vp, vp, vp, vp, vp, vp]
     L.tj_l3_range.argtypes = [ci, ci, ci, ci, ip, ip, ip]
     L.tj_sweep_counts.argtypes = [ci, ci, ci, ip, ip, ip, ip]
@@ -215,6 +216,26 @@ def coupling_multi(tables: Tables, Wtt, Wtp, Wpp, want=_BLOCKS, out=None, stream
     _check(load_library().tj_coupling_multi(tables.handle, nwin, _dev_ptr(Wtt, nwin * nW, "Wtt"),
                                             _dev_ptr(Wtp, nwin * nW, "Wtp"), _dev_ptr(Wpp, nwin * nW, "Wpp"), nW,
                                             *args, _stream_ptr(stream)), "tj_coupling_multi")
+    return {k: out[k] for k in want}
+
+
+_SPIN1 = ("K00", "K01", "K11p", "K11m")
+
+
+def coupling_spin1(tables: Tables, W00, W01, W11, want=_SPIN1, out=None, stream=None):
+    """tj_coupling_spin1.  Returns dict name -> [(lmax+1),(lmax+1)] tensor for the blocks in `want`."""
+    import torch
+    N = tables.lmax + 1
+    nW = tables.l3max + 1
+    dev = next(w for w in (W00, W01, W11) if w is not None).device
+    out = {} if out is None else dict(out)
+    for k in want:
+        if k not in out:
+            out[k] = torch.empty((N, N), dtype=torch.float64, device=dev)
+    args = [_dev_ptr(out.get(k) if k in want else None, N * N, k) for k in _SPIN1]
+    _check(load_library().tj_coupling_spin1(tables.handle, _dev_ptr(W00, nW, "W00"), _dev_ptr(W01, nW, "W01"),
+                                            _dev_ptr(W11, nW, "W11"), nW, *args, _stream_ptr(stream)),
+           "tj_coupling_spin1")
     return {k: out[k] for k in want}
 
 

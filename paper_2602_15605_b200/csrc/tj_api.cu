@@ -70,6 +70,7 @@ struct Call {
     bool banded = false;
     int lcut = -1, mask = 0, R = 0, l3max_eff = 0, nb = 0, ntiles = 0, ntile_w = 0;
     int nw = 1;                     // window sets per sweep (tj_coupling_multi: 2)
+    int spin = 2;                   // 2: TT/TE/EE/EB; 1: K00/K01/K11+/K11- in the same slots (tj_coupling_spin1)
     int nW = 0;                     // entries per window
     long long N = 0, ld = 0;
     double *TT = nullptr, *TE = nullptr, *ee = nullptr, *EB = nullptr, *bb_copy = nullptr;
@@ -80,7 +81,8 @@ struct Call {
 
 // One coupling call on device pointers.  lcut < 0: dense (l3max = handle's); else banded with l3 <= lcut.
 int run_coupling(const tj_tables *tables, int lcut, const double *d_Wtt, const double *d_Wtp, const double *d_Wpp,
-                 int nW, double *d_TT, double *d_TE, double *d_EE, double *d_BB, double *d_EB, cudaStream_t st, int nw = 1);
+                 int nW, double *d_TT, double *d_TE, double *d_EE, double *d_BB, double *d_EB, cudaStream_t st, int nw = 1,
+                 int spin = 2);
 int run_coupling_rows_to_host(const tj_tables *tables, const double *d_Wtt, const double *d_Wtp, const double *d_Wpp,
                               int nW, double *const d_out[5], double *const h_out[5], cudaStream_t st);
 
@@ -117,7 +119,7 @@ int tj_build_tables(int lmax, int l3max, void *cuda_stream, tj_tables **out)
     T.pmax = 2 * lmax + 1;
     T.np_alloc = GUARD_LO + T.pmax + 1 + GUARD_HI;
     T.nl_alloc = GUARD_LO + 2 * lmax + 2 + GUARD_HI;   // even, like np_alloc: every table's index 0 is 16-byte aligned (bulk copies)
-    size_t n = (size_t)5 * T.np_alloc + (size_t)2 * T.nl_alloc;
+    size_t n = (size_t)5 * T.np_alloc + (size_t)3 * T.nl_alloc;
     cudaError_t e = cudaMalloc((void **)&T.base, n * sizeof(double));
     if (e != cudaSuccess) { delete h; return cuda_fail(e, "tj_build_tables/cudaMalloc"); }
     double *p = T.base + GUARD_LO;
@@ -127,7 +129,8 @@ int tj_build_tables(int lmax, int l3max, void *cuda_stream, tj_tables **out)
     T.gA = p;   p += T.np_alloc;
     T.gB = p;   p += T.np_alloc;
     T.u3 = p;   p += T.nl_alloc;
-    T.isd = p;
+    T.isd = p;  p += T.nl_alloc;
+    T.isu = p;
     e = launch_build_tables(T, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
     if (e != cudaSuccess) { cudaFree(T.base); delete h; return cuda_fail(e, "tj_build_tables"); }
@@ -166,6 +169,7 @@ int tj_tables_copy(const tj_tables *tables, int which, double *h_dst, int count)
         case 4: src = T.gB; maxn = T.pmax + 1; break;
         case 5: src = T.u3; maxn = T.lmax + 1; break;
         case 6: src = T.isd; maxn = T.lmax + 1; break;
+        case 7: src = T.isu; maxn = T.lmax + 1; break;
         default: return TJ_EINVAL;
     }
     if (count > maxn) return TJ_EINVAL;
@@ -218,6 +222,16 @@ int tj_coupling_multi(const tj_tables *tables, int nwin, const double *d_Wtt, co
         w += nw;
     }
     return TJ_OK;
+}
+
+int tj_coupling_spin1(const tj_tables *tables, const double *d_W00, const double *d_W01, const double *d_W11, int nW,
+                      double *d_K00, double *d_K01, double *d_K11p, double *d_K11m, void *cuda_stream)
+{
+    if (!tables) return TJ_EINVAL;
+    if (nW != tables->T.l3max + 1) return TJ_EINVAL;
+    // same sweep, spin-1 algebra: K00 rides in the TT slot, K01 in TE, K11+ in EE, K11- in EB
+    return run_coupling(tables, -1, d_W00, d_W01, d_W11, nW, d_K00, d_K01, d_K11p, nullptr, d_K11m,
+                        (cudaStream_t)cuda_stream, 1, 1);
 }
 
 int tj_coupling_host(const tj_tables *tables, int band, int nW_or_lcut, const double *h_Wtt, const double *h_Wtp,
@@ -375,11 +389,12 @@ namespace {
 // ---- one coupling call, in pieces (the host-buffer path launches the middle two per row chunk) -------------
 int coupling_begin(Call &C, const tj_tables *tables, int lcut, const double *d_Wtt, const double *d_Wtp,
                    const double *d_Wpp, int nW, double *d_TT, double *d_TE, double *d_EE, double *d_BB, double *d_EB,
-                   cudaStream_t st, int nw = 1)
+                   cudaStream_t st, int nw = 1, int spin = 2)
 {
     const Tables &T = tables->T;
     C.T = &T;
     C.nw = nw;
+    C.spin = spin;
     C.nW = nW;
     C.banded = lcut >= 0;
     C.lcut = lcut;
@@ -446,7 +461,8 @@ cudaError_t coupling_sweep(const Call &C, int b0, int b1, cudaStream_t st)
 {
     const Tables &T = *C.T;
     SweepParams P;
-    P.g = T.g; P.ginv = T.ginv; P.h = T.h; P.gA = T.gA; P.gB = T.gB; P.u3 = T.u3; P.isd = T.isd;
+    P.g = T.g; P.ginv = T.ginv; P.h = T.h; P.gA = T.gA; P.gB = T.gB; P.u3 = T.u3;
+    P.isd = C.spin == 1 ? T.isu : T.isd;
     P.wtt = C.wtt; P.wtp = C.wtp; P.wpp = C.wpp;
     // a block the instantiated sweep computes but the caller did not ask for has a NULL target and is not stored
     P.TT = C.TT; P.TE = C.TE; P.EE = C.ee; P.EB = C.EB;
@@ -457,7 +473,7 @@ cudaError_t coupling_sweep(const Call &C, int b0, int b1, cudaStream_t st)
     P.wstride = 3 * (long long)T.nl_alloc;
     P.ostride = C.N * C.ld;
     const int n = all ? C.ntiles : tiles_above(C, b0 - 1) - P.tile_off;
-    return launch_sweep(P, C.mask, C.nw, n, st);
+    return launch_sweep(P, C.mask, C.nw, C.mask == M_TT ? 2 : C.spin, n, st);
 }
 
 // scale + mirror of the 32-row tile rows [I0, I1)
@@ -493,10 +509,11 @@ void coupling_end(Call &C, cudaStream_t st)
 }
 
 int run_coupling(const tj_tables *tables, int lcut, const double *d_Wtt, const double *d_Wtp, const double *d_Wpp,
-                 int nW, double *d_TT, double *d_TE, double *d_EE, double *d_BB, double *d_EB, cudaStream_t st, int nw)
+                 int nW, double *d_TT, double *d_TE, double *d_EE, double *d_BB, double *d_EB, cudaStream_t st, int nw,
+                 int spin)
 {
     Call C;
-    int rc = coupling_begin(C, tables, lcut, d_Wtt, d_Wtp, d_Wpp, nW, d_TT, d_TE, d_EE, d_BB, d_EB, st, nw);
+    int rc = coupling_begin(C, tables, lcut, d_Wtt, d_Wtp, d_Wpp, nW, d_TT, d_TE, d_EE, d_BB, d_EB, st, nw, spin);
     if (rc != TJ_OK) return rc;
     prof_record(2, st);
     cudaError_t e = coupling_sweep(C, 0, C.nb, st);

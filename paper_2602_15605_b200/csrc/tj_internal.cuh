@@ -57,6 +57,7 @@ struct Tables {
     double *g, *ginv, *h, *gA, *gB; // p-indexed
     double *u3;                     // l-indexed: u3[l] = l(l+1)
     double *isd;                    // l-indexed: 1/sqrt(D_l), 0 for l < 2
+    double *isu;                    // l-indexed: 1/sqrt(u_l), 0 for l < 1 (spin-1 blocks)
 };
 
 struct SweepParams {
@@ -89,7 +90,7 @@ cudaError_t launch_prepare(const Tables &T, const double *d_Wtt, const double *d
                            double *wtt, double *wtp, double *wpp, int *tile_start, int R, int l3max_eff, bool banded,
                            cudaStream_t st);
 int sweep_R(int mask, bool banded, int nw);   // pairs per thread (= rows per band) of the sweep that serves `mask` for nw window sets
-cudaError_t launch_sweep(const SweepParams &P, int mask, int nw, int total_tiles, cudaStream_t st);
+cudaError_t launch_sweep(const SweepParams &P, int mask, int nw, int spin, int total_tiles, cudaStream_t st);
 cudaError_t launch_writer(const WriterParams &P, cudaStream_t st);
 cudaError_t launch_fp64_probe(int iters, double *d_sink, int blocks, int threads, cudaStream_t st);
 

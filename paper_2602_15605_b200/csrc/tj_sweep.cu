@@ -115,7 +115,11 @@ __device__ __forceinline__ int slice_bytes(int i0, int n)
     return ((n + (i0 - ie) + 1) & ~1) * 8;
 }
 
-template <int R, int MASK, int TS, int MINB, bool PIPE, int NW>
+// SPIN = 2: the paper's blocks (above).  SPIN = 1: the same sweep with the (l1 l2 l3;-1 1 0) symbol
+// (DESIGN.md 3 item 6):  even step: (-1 1 0) = X d / (2 sqrt(u1 u2)), d = u3-u1-u2, so the
+// "TE" slot accumulates W' X^2 d and the "EE" slot W' X^2 d^2; odd step: (-1 1 0)^2 = Z^2 / (4 u1 u2), so the "EB"
+// slot accumulates W' Z^2; P.isd then holds 1/sqrt(u_l) and the epilogue scales are the same expressions.
+template <int R, int MASK, int TS, int MINB, bool PIPE, int NW, int SPIN>
 __global__ void __launch_bounds__(SWEEP_THREADS, MINB) sweep_tma_kernel(const __grid_constant__ SweepParams P)
 {
     constexpr bool kTT = (MASK & M_TT) != 0, kTE = (MASK & M_TE) != 0, kEE = (MASK & M_EE) != 0,
@@ -216,8 +220,8 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB) sweep_tma_kernel(const __
         for (int i = 0; i < R; ++i) {
             const double l1 = (double)(a + i), l2 = (double)(c - i);
             const double u1 = l1 * (l1 + 1.0), u2 = l2 * (l2 + 1.0);
-            c12[i] = u1 + u2 - 2.0;                  // odd branch: e = u3 - c12
-            kk[i] = __fma_rn(2.0 * u1, u2, 1.0);     // even branch: A2 = d1^2 - kk
+            c12[i] = SPIN == 2 ? u1 + u2 - 2.0 : u1 + u2 - 1.0;   // odd branch: e = u3 - c12 (spin 1: unused)
+            kk[i] = __fma_rn(2.0 * u1, u2, 1.0);     // even branch: A2 = d1^2 - kk (spin 1: unused)
         }
     }
 
@@ -275,12 +279,14 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB) sweep_tma_kernel(const __
                         double r[R], e[R];
 #pragma unroll
                         for (int i = 0; i < R; ++i) r[i] = __dmul_rn(wa[(i - u + R) % R], wb[(2 * R - i - u) % R]);
+                        if (SPIN == 2) {
 #pragma unroll
-                        for (int i = 0; i < R; ++i) e[i] = __dsub_rn(c3, c12[i]);
+                            for (int i = 0; i < R; ++i) e[i] = __dsub_rn(c3, c12[i]);
 #pragma unroll
-                        for (int i = 0; i < R; ++i) r[i] = __dmul_rn(r[i], e[i]);
+                            for (int i = 0; i < R; ++i) r[i] = __dmul_rn(r[i], e[i]);
 #pragma unroll
-                        for (int i = 0; i < R; ++i) r[i] = __dmul_rn(r[i], e[i]);
+                            for (int i = 0; i < R; ++i) r[i] = __dmul_rn(r[i], e[i]);
+                        }
 #pragma unroll
                         for (int w = 0; w < NW; ++w)
 #pragma unroll
@@ -412,8 +418,10 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB) sweep_tma_kernel(const __
                         if (kA2) {
 #pragma unroll
                             for (int i = 0; i < R; ++i) A2[i] = __dsub_rn(c3, c12[i]);
+                            if (SPIN == 2) {
 #pragma unroll
-                            for (int i = 0; i < R; ++i) A2[i] = __fma_rn(A2[i], A2[i], -kk[i]);
+                                for (int i = 0; i < R; ++i) A2[i] = __fma_rn(A2[i], A2[i], -kk[i]);
+                            }
 #pragma unroll
                             for (int i = 0; i < R; ++i) rA[i] = __dmul_rn(r[i], A2[i]);
                             if (kEE) {
@@ -472,7 +480,7 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB) sweep_tma_kernel(const __
     }
 }
 
-template <int R, int MASK, int TS, int MINB, bool PIPE, int NW = 1>
+template <int R, int MASK, int TS, int MINB, bool PIPE, int NW = 1, int SPIN = 2>
 cudaError_t launch_one(const SweepParams &P, int total_tiles, cudaStream_t st)
 {
     if (total_tiles <= 0) return cudaSuccess;
@@ -480,12 +488,12 @@ cudaError_t launch_one(const SweepParams &P, int total_tiles, cudaStream_t st)
     constexpr size_t smem = (size_t)NWARP * NBUF * Lay<TS, NW>::BUFD * 8 + (size_t)NWARP * NBUF * 8;
     static bool attr_set = false;   // per instantiation
     if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(sweep_tma_kernel<R, MASK, TS, MINB, PIPE, NW>,
+        cudaError_t e = cudaFuncSetAttribute(sweep_tma_kernel<R, MASK, TS, MINB, PIPE, NW, SPIN>,
                                              cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         attr_set = true;
     }
-    sweep_tma_kernel<R, MASK, TS, MINB, PIPE, NW><<<total_tiles, SWEEP_THREADS, smem, st>>>(P);
+    sweep_tma_kernel<R, MASK, TS, MINB, PIPE, NW, SPIN><<<total_tiles, SWEEP_THREADS, smem, st>>>(P);
     return cudaGetLastError();
 }
 
@@ -504,10 +512,15 @@ int sweep_R(int mask, bool banded, int nw)
     return banded ? R_POL_BAND : R_POL;
 }
 
-cudaError_t launch_sweep(const SweepParams &P, int mask, int nw, int total_tiles, cudaStream_t st)
+cudaError_t launch_sweep(const SweepParams &P, int mask, int nw, int spin, int total_tiles, cudaStream_t st)
 {
     constexpr int POL = M_TE | M_EE | M_EB, ALL = M_TT | POL;
     const bool banded = P.lcut >= 0;
+    if (spin == 1) {   // dense, one window set; TT-only requests use the spin-independent TT sweep below
+        if (banded || nw != 1) return cudaErrorInvalidValue;
+        if (mask == ALL) return launch_one<R_POL, ALL, TS_DENSE_SHORT, 2, true, 1, 1>(P, total_tiles, st);
+        if (mask == POL) return launch_one<R_POL, POL, TS_DENSE_SHORT, 2, true, 1, 1>(P, total_tiles, st);
+    }
     if (nw == 2 && !banded && mask == ALL) return launch_one<R_MULTI2, ALL, 48, 2, true, 2>(P, total_tiles, st);
     if (nw != 1) return cudaErrorInvalidValue;
     switch (mask) {

@@ -123,6 +123,7 @@ __global__ void build_ltables_kernel(Tables T)
         double u = dl * (dl + 1.0);
         T.u3[l] = u;
         T.isd[l] = (l >= 2 && l <= T.lmax) ? 1.0 / sqrt(u * (u - 2.0)) : 0.0;
+        T.isu[l] = (l >= 1 && l <= T.lmax) ? 1.0 / sqrt(u) : 0.0;
     }
 }
 
@@ -131,7 +132,7 @@ __global__ void build_ltables_kernel(Tables T)
 cudaError_t launch_build_tables(const Tables &T, cudaStream_t st)
 {
     // guards and the tail beyond pmax are zero: one memset of the whole allocation
-    size_t bytes = sizeof(double) * ((size_t)5 * T.np_alloc + (size_t)2 * T.nl_alloc);
+    size_t bytes = sizeof(double) * ((size_t)5 * T.np_alloc + (size_t)3 * T.nl_alloc);
     cudaError_t e = cudaMemsetAsync(T.base, 0, bytes, st);
     if (e != cudaSuccess) return e;
     build_tables_kernel<<<1, TB_THREADS, 0, st>>>(T);
