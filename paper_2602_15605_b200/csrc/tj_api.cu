@@ -409,7 +409,7 @@ int coupling_begin(Call &C, const tj_tables *tables, int lcut, const double *d_W
     if (!d_TE && !C.ee && !d_EB) C.mask = M_TT;
     else if (d_TT) C.mask = M_TT | M_TE | M_EE | M_EB;
     else C.mask = M_TE | M_EE | M_EB;
-    C.R = sweep_R(C.mask, C.banded, nw);
+    C.R = sweep_R(C.mask, C.banded, nw, T.lmax);
     C.l3max_eff = C.banded ? lcut : T.l3max;
     C.N = (long long)T.lmax + 1;
     C.ld = C.banded ? (long long)(2 * lcut + 1) : C.N;

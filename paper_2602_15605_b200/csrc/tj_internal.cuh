@@ -22,7 +22,9 @@ constexpr int GUARD_HI = 768;
 constexpr int SWEEP_THREADS = 128;   // columns c per CTA
 constexpr int R_POL = 12;           // pairs per thread, fused TT+TE+EE(+EB) sweep, dense storage
 constexpr int R_POL_BAND = 8;       // same, band-limited (short sweeps)
-constexpr int R_TT = 16;             // pairs per thread, TT-only sweep
+constexpr int R_TT = 16;            // pairs per thread, TT-only sweep (short or band-limited sweeps)
+constexpr int R_TT_LONG = 32;       // same, dense sweeps at lmax >= LMAX_LONG (measured at lmax = 10^4: 24.9 -> 22.8 ms)
+constexpr int LMAX_LONG = 4096;     // from here on a dense sweep uses the long-sweep geometry (R_TT_LONG; 96-step stages)
 constexpr int R_MULTI2 = 8;         // pairs per thread, 2 window sets per sweep (tj_coupling_multi)
 
 // mask bits of the blocks one sweep computes
@@ -89,7 +91,7 @@ cudaError_t launch_build_tables(const Tables &T, cudaStream_t st);
 cudaError_t launch_prepare(const Tables &T, const double *d_Wtt, const double *d_Wtp, const double *d_Wpp, int nW,
                            double *wtt, double *wtp, double *wpp, int *tile_start, int R, int l3max_eff, bool banded,
                            cudaStream_t st);
-int sweep_R(int mask, bool banded, int nw);   // pairs per thread (= rows per band) of the sweep that serves `mask` for nw window sets
+int sweep_R(int mask, bool banded, int nw, int lmax);   // pairs per thread (= rows per band) of the sweep that serves `mask` for nw window sets
 cudaError_t launch_sweep(const SweepParams &P, int mask, int nw, int spin, int total_tiles, cudaStream_t st);
 cudaError_t launch_writer(const WriterParams &P, cudaStream_t st);
 cudaError_t launch_fp64_probe(int iters, double *d_sink, int blocks, int threads, cudaStream_t st);

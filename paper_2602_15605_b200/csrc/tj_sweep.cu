@@ -55,7 +55,6 @@ namespace {
 // turn-over (measured at lmax = 10^4: TS = 24 148.8 ms, 48 143.4 ms, 96 141.7 ms) but round every warp's walk
 // up to whole stages, so short sweeps keep the short stage
 constexpr int TS_DENSE_LONG = 96, TS_DENSE_SHORT = 48;
-constexpr int LMAX_LONG_STAGES = 4096;
 constexpr int NBUF = 2;   // buffers per warp
 constexpr int PAD = 2;    // doubles in front of each slice: the software-pipelined read of "step TS" lands here
 
@@ -505,10 +504,10 @@ cudaError_t launch_one(const SweepParams &P, int total_tiles, cudaStream_t st)
 // Multi-window batching (nw window sets in one sweep): the geometric part of a term (r, A2, rA, rAA) is
 // computed once and each window set adds 3 FMAs (1 in the odd branch); the accumulators of nw sets take the
 // registers that R = 12 pairs use otherwise, hence R = 8 for nw = 2 (the only batched instantiation).
-int sweep_R(int mask, bool banded, int nw)
+int sweep_R(int mask, bool banded, int nw, int lmax)
 {
     if (nw == 2) return R_MULTI2;
-    if (mask == M_TT) return R_TT;
+    if (mask == M_TT) return (!banded && lmax >= LMAX_LONG) ? R_TT_LONG : R_TT;
     return banded ? R_POL_BAND : R_POL;
 }
 
@@ -526,14 +525,15 @@ cudaError_t launch_sweep(const SweepParams &P, int mask, int nw, int spin, int t
     switch (mask) {
         case M_TT:
             return banded ? launch_one<R_TT, M_TT, 32, 3, false>(P, total_tiles, st)
-                          : launch_one<R_TT, M_TT, 48, 3, false>(P, total_tiles, st);
+                          : (P.lmax >= LMAX_LONG ? launch_one<R_TT_LONG, M_TT, 64, 2, false>(P, total_tiles, st)
+                                                 : launch_one<R_TT, M_TT, 48, 3, false>(P, total_tiles, st));
         case POL:
             return banded ? launch_one<R_POL_BAND, POL, 32, 3, false>(P, total_tiles, st)
-                          : (P.lmax >= LMAX_LONG_STAGES ? launch_one<R_POL, POL, TS_DENSE_LONG, 2, true>(P, total_tiles, st)
+                          : (P.lmax >= LMAX_LONG ? launch_one<R_POL, POL, TS_DENSE_LONG, 2, true>(P, total_tiles, st)
                                                         : launch_one<R_POL, POL, TS_DENSE_SHORT, 2, true>(P, total_tiles, st));
         case ALL:
             return banded ? launch_one<R_POL_BAND, ALL, 32, 3, false>(P, total_tiles, st)
-                          : (P.lmax >= LMAX_LONG_STAGES ? launch_one<R_POL, ALL, TS_DENSE_LONG, 2, true>(P, total_tiles, st)
+                          : (P.lmax >= LMAX_LONG ? launch_one<R_POL, ALL, TS_DENSE_LONG, 2, true>(P, total_tiles, st)
                                                         : launch_one<R_POL, ALL, TS_DENSE_SHORT, 2, true>(P, total_tiles, st));
         default: return cudaErrorInvalidValue;
     }

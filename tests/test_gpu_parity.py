@@ -490,3 +490,21 @@ def test_spin1_config1_sampled_rows():
         # Xi symmetry through the mirrored writer
         a = got[k] * (2.0 * np.arange(N)[:, None] + 1.0)
         assert np.allclose(a, a.T, rtol=1e-15, atol=0)
+
+
+@pytest.mark.parametrize("lmax", [4095, 4096, 5000])
+def test_tt_only_long_geometry(lmax):
+    """tj_coupling_tt switches to R = 32 pairs per thread at lmax >= 4096: sampled entries against the
+    oracle, and the whole matrix bitwise against the TT block of the fused sweep (same operations per entry)."""
+    import torch
+    wl = windows.config(2, lmax=lmax)
+    T = binding.build_tables(wl.lmax)
+    TT = binding.coupling_tt(T, _t(wl.Wtt))
+    pol = binding.coupling_pol(T, _t(wl.Wtt), _t(wl.Wtp), _t(wl.Wpp), want=("TT", "TE", "EE", "EB"))
+    torch.cuda.synchronize()
+    assert torch.equal(TT, pol["TT"])
+    l1, l2 = _sample_pairs(wl.lmax, 1500, 300 + lmax)
+    ref = oracle.coupling_pairs(wl.l3max, wl.Wtt, None, None, l1, l2)
+    got = TT[torch.as_tensor(l1.astype(np.int64)).cuda(), torch.as_tensor(l2.astype(np.int64)).cuda()].cpu().numpy()
+    assert_parity(got, ref["TT"], "TT-only lmax=%d" % lmax)
+    T.close()
