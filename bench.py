@@ -168,6 +168,8 @@ def main():
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json configs index (headline: 3)")
     ap.add_argument("--nwin", type=int, default=1,
                     help="window sets per step through tj_coupling_multi (default 1: the headline tj_coupling_pol step)")
+    ap.add_argument("--ablation", action="store_true",
+                    help="also time tj_coupling_literal (the paper's per-pair Eq. 10 / Eq. 16 evaluation) on the same workload")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
@@ -335,6 +337,21 @@ def main():
                "ms_per_step": 1e3 * dt / n_e2e, "steps": n_e2e, "api": "tj_coupling_host (pinned host buffers)"}
         del hout
 
+    ablation = None
+    if args.ablation and wl.pol and not wl.band and nwin == 1:
+        # the paper's own design on this GPU (tj_literal.cu): one thread per pair, Eq. 10 (TT) / Eq. 16 literally (EE)
+        ablation = {"kernel": "literal_kernel (one thread per (l1,l2), PAPER.md:240; Eq. 10 / Eq. 16)", "unit": "ms"}
+        for name, a in (("TT", (dW[0], None, ("TT",))), ("EE", (None, dW[2], ("EE",)))):
+            binding.coupling_literal(T, a[0], a[1], want=a[2])
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            binding.coupling_literal(T, a[0], a[1], want=a[2])
+            e1.record()
+            torch.cuda.synchronize()
+            ablation[name] = e0.elapsed_time(e1)
+        ablation["note"] = "fused sweep of this line: all five blocks in %.1f ms" % sweep_ms
+
     cpu_baseline = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline and not wl.band:
         cpu_baseline = time_oracle(wl, args.config)
@@ -349,7 +366,7 @@ def main():
                        "pairs_per_s": world * P * args.steps / (total_ms * 1e-3),
                        "l2": "512 MB flush written between timed steps; each step also writes %.1f GB of output" % (bytes_out / 1e9),
                        "parallelism": "1 problem per GPU" if world > 1 else "single GPU"},
-            "roofline": roofline, "cpu_baseline": cpu_baseline, "e2e": e2e,
+            "roofline": roofline, "cpu_baseline": cpu_baseline, "e2e": e2e, "ablation": ablation,
             # a batched pair of window sets: 2 prepare + 1 sweep + 2 writer launches; a single set: 3
             "gpu_launches": ((nwin // 2) * 5 + (nwin % 2) * 3) * args.steps if nwin > 1
             else binding.launches_per_call(1) * args.steps,

@@ -123,6 +123,19 @@ int tj_coupling_spin1(const tj_tables *tables,
                       void *cuda_stream);
 
 /*
+ * tj_coupling_literal -- ABLATION, not the hot path: the paper's own evaluation restated as
+ * one plain kernel -- one thread per (l1,l2) of the upper triangle, serial l3 loop in steps of 2 with direct
+ * table lookups, K^{TT} from Eq. 10 and K^{EE} from Eq. 16
+ * evaluated literally (PAPER.md:216-220 with alpha, beta, eta of Eqs. B14-B16: two table
+ * products and two square roots per term), mirrored into the lower triangle.  It exists so
+ * that the paper's cost structure (EE ~ 5x TT) and its GPU design can be timed on this GPU
+ * beside the fused sweep; results agree with tj_coupling_pol to rounding (~1e-12).
+ *   d_TT / d_EE: (lmax+1)^2 doubles, either may be NULL (with its window).  Windows: nW = l3max+1 entries.
+ */
+int tj_coupling_literal(const tj_tables *tables, const double *d_Wtt, const double *d_Wpp, int nW,
+                        double *d_TT, double *d_EE, void *cuda_stream);
+
+/*
  * Host-buffer forms (the end-to-end path): same semantics, but every window and output is a HOST
  * pointer (h_*; pinned memory makes the copies asynchronous and fast, pageable memory also works).
  * The call allocates device scratch from the stream-ordered pool, copies the windows in, runs the same

@@ -18,7 +18,7 @@ TJ_OK, TJ_EINVAL, TJ_ENOMEM, TJ_ECUDA = 0, -1, -2, -3
 # every symbol include/tj.h declares (tests/test_abi.py checks the header against this and the .so)
 SYMBOLS = (
     "tj_build_tables", "tj_free_tables", "tj_tables_info", "tj_tables_copy",
-    "tj_coupling_tt", "tj_coupling_pol", "tj_coupling_band", "tj_coupling_multi", "tj_coupling_spin1", "tj_coupling_host",
+    "tj_coupling_tt", "tj_coupling_pol", "tj_coupling_band", "tj_coupling_multi", "tj_coupling_spin1", "tj_coupling_literal", "tj_coupling_host",
     "tj_l3_range", "tj_sweep_counts", "tj_fp64_probe", "tj_profile_enable", "tj_profile_get",
     "tj_launches_per_call", "tj_strerror",
 )
@@ -54,6 +54,7 @@ def load_library() -> ctypes.CDLL:
     L.tj_coupling_band.argtypes = [vp, ci, vp, vp, vp, vp, vp, vp, vp, vp, vp]
     L.tj_coupling_multi.argtypes = [vp, ci, vp, vp, vp, ci, vp, vp, vp, vp, vp, vp]
     L.tj_coupling_spin1.argtypes = [vp, vp, vp, vp, ci, vp, vp, vp, vp, vp]
+    L.tj_coupling_literal.argtypes = [vp, vp, vp, ci, vp, vp, vp]
     L.tj_coupling_host.argtypes = [vp, ci, ci, vp, vp, vp, vp, vp, vp, vp, vp, vp]
     L.tj_l3_range.argtypes = [ci, ci, ci, ci, ip, ip, ip]
     L.tj_sweep_counts.argtypes = [ci, ci, ci, ip, ip, ip, ip]
@@ -237,6 +238,19 @@ def coupling_spin1(tables: Tables, W00, W01, W11, want=_SPIN1, out=None, stream=
                                             _dev_ptr(W11, nW, "W11"), nW, *args, _stream_ptr(stream)),
            "tj_coupling_spin1")
     return {k: out[k] for k in want}
+
+
+def coupling_literal(tables: Tables, Wtt, Wpp, want=("TT", "EE"), stream=None):
+    """tj_coupling_literal (ablation: the paper's own per-pair evaluation, Eq. 10 / Eq. 16 literally)."""
+    import torch
+    N = tables.lmax + 1
+    nW = tables.l3max + 1
+    dev = next(w for w in (Wtt, Wpp) if w is not None).device
+    out = {k: torch.empty((N, N), dtype=torch.float64, device=dev) for k in want}
+    _check(load_library().tj_coupling_literal(tables.handle, _dev_ptr(Wtt, nW, "Wtt"), _dev_ptr(Wpp, nW, "Wpp"), nW,
+                                              _dev_ptr(out.get("TT"), N * N, "TT"), _dev_ptr(out.get("EE"), N * N, "EE"),
+                                              _stream_ptr(stream)), "tj_coupling_literal")
+    return out
 
 
 def coupling_host(tables: Tables, Wtt, Wtp, Wpp, out: dict, band_lcut: int | None = None, stream=None):

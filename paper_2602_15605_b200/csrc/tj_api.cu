@@ -85,6 +85,8 @@ int run_coupling(const tj_tables *tables, int lcut, const double *d_Wtt, const d
                  int spin = 2);
 int run_coupling_rows_to_host(const tj_tables *tables, const double *d_Wtt, const double *d_Wtp, const double *d_Wpp,
                               int nW, double *const d_out[5], double *const h_out[5], cudaStream_t st);
+int run_literal(const tj_tables *tables, const double *d_Wtt, const double *d_Wpp, int nW, double *d_TT, double *d_EE,
+                cudaStream_t st);
 
 }  // namespace
 
@@ -232,6 +234,16 @@ int tj_coupling_spin1(const tj_tables *tables, const double *d_W00, const double
     // same sweep, spin-1 algebra: K00 rides in the TT slot, K01 in TE, K11+ in EE, K11- in EB
     return run_coupling(tables, -1, d_W00, d_W01, d_W11, nW, d_K00, d_K01, d_K11p, nullptr, d_K11m,
                         (cudaStream_t)cuda_stream, 1, 1);
+}
+
+int tj_coupling_literal(const tj_tables *tables, const double *d_Wtt, const double *d_Wpp, int nW, double *d_TT,
+                        double *d_EE, void *cuda_stream)
+{
+    if (!tables || (!d_TT && !d_EE)) return TJ_EINVAL;
+    if (nW != tables->T.l3max + 1) return TJ_EINVAL;
+    if ((d_TT && !d_Wtt) || (d_EE && !d_Wpp)) return TJ_EINVAL;
+    if (tables->T.lmax > 65534) return TJ_EINVAL;   // grid.y = lmax+1
+    return run_literal(tables, d_Wtt, d_Wpp, nW, d_TT, d_EE, (cudaStream_t)cuda_stream);
 }
 
 int tj_coupling_host(const tj_tables *tables, int band, int nW_or_lcut, const double *h_Wtt, const double *h_Wtp,
@@ -524,6 +536,19 @@ int run_coupling(const tj_tables *tables, int lcut, const double *d_Wtt, const d
     coupling_end(C, st);
     return rc;
 }
+// paper-literal ablation (tj_literal.cu): prefold the windows, then one thread per pair
+int run_literal(const tj_tables *tables, const double *d_Wtt, const double *d_Wpp, int nW, double *d_TT, double *d_EE,
+                cudaStream_t st)
+{
+    Call C;
+    int rc = coupling_begin(C, tables, -1, d_Wtt, nullptr, d_Wpp, nW, d_TT, nullptr, d_EE, nullptr, nullptr, st);
+    if (rc != TJ_OK) return rc;
+    cudaError_t e = launch_literal(*C.T, C.wtt, C.wpp, d_TT, d_EE, C.l3max_eff, st);
+    if (e != cudaSuccess) rc = cuda_fail(e, "tj_coupling_literal");
+    coupling_end(C, st);
+    return rc;
+}
+
 // ---- dense call with HOST outputs, pipelined by row chunks ------------------------------------------------
 // Full row l1 of a matrix is final once (i) the sweep and writer of its own row band have run (upper part
 // and diagonal) and (ii) the writers of every band above it have run (they store the mirrored lower part).

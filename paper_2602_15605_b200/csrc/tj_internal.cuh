@@ -94,6 +94,8 @@ cudaError_t launch_prepare(const Tables &T, const double *d_Wtt, const double *d
 int sweep_R(int mask, bool banded, int nw, int lmax);   // pairs per thread (= rows per band) of the sweep that serves `mask` for nw window sets
 cudaError_t launch_sweep(const SweepParams &P, int mask, int nw, int spin, int total_tiles, cudaStream_t st);
 cudaError_t launch_writer(const WriterParams &P, cudaStream_t st);
+cudaError_t launch_literal(const Tables &T, const double *wtt, const double *wpp, double *TT, double *EE, int l3max,
+                           cudaStream_t st);   // paper-literal ablation kernel (tj_literal.cu)
 cudaError_t launch_fp64_probe(int iters, double *d_sink, int blocks, int threads, cudaStream_t st);
 
 }  // namespace tj

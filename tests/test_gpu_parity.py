@@ -508,3 +508,31 @@ def test_tt_only_long_geometry(lmax):
     got = TT[torch.as_tensor(l1.astype(np.int64)).cuda(), torch.as_tensor(l2.astype(np.int64)).cuda()].cpu().numpy()
     assert_parity(got, ref["TT"], "TT-only lmax=%d" % lmax)
     T.close()
+
+
+# ---------------------------------------------------------------- paper-literal ablation kernel
+def test_literal_eq16_kernel_against_oracle_and_sweep():
+    import torch
+    for lmax, l3max in ((150, 300), (97, 120)):
+        wl = windows.config(1, lmax=lmax)
+        Wtt, Wpp = wl.Wtt[: l3max + 1], wl.Wpp[: l3max + 1]
+        T = binding.build_tables(lmax, l3max)
+        lit = binding.coupling_literal(T, _t(Wtt), _t(Wpp))
+        torch.cuda.synchronize()
+        ref = oracle.coupling_full(lmax, l3max, Wtt, None, Wpp)
+        assert_parity(lit["TT"].cpu().numpy(), ref["TT"], "literal TT lmax=%d" % lmax)
+        assert_parity(lit["EE"].cpu().numpy(), ref["EE"], "literal EE lmax=%d" % lmax)
+        T.close()
+    wl = windows.config(1)
+    T = binding.build_tables(wl.lmax)
+    lit = binding.coupling_literal(T, _t(wl.Wtt), _t(wl.Wpp))
+    pol = binding.coupling_pol(T, _t(wl.Wtt), None, _t(wl.Wpp), want=("TT", "EE"))
+    torch.cuda.synchronize()
+    for k in ("TT", "EE"):
+        a, b = lit[k], pol[k]
+        rel = ((a - b).abs() / b.abs().clamp_min(1e-300))[b.abs() >= SMALL]
+        assert float(rel.max()) < 1e-10, (k, float(rel.max()))
+        print("literal vs fused sweep, cfg1 %s: worst rel %.2e" % (k, float(rel.max())))
+    only = binding.coupling_literal(T, None, _t(wl.Wpp), want=("EE",))
+    assert torch.equal(only["EE"], lit["EE"])
+    T.close()
