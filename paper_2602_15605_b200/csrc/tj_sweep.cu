@@ -55,6 +55,9 @@ namespace {
 // turn-over (measured at lmax = 10^4: TS = 24 148.8 ms, 48 143.4 ms, 96 141.7 ms) but round every warp's walk
 // up to whole stages, so short sweeps keep the short stage
 constexpr int TS_DENSE_LONG = 96, TS_DENSE_SHORT = 48;
+#ifndef TJ_TS_BAND
+#define TJ_TS_BAND 32
+#endif
 constexpr int NBUF = 2;   // buffers per warp
 constexpr int PAD = 2;    // doubles in front of each slice: the software-pipelined read of "step TS" lands here
 
@@ -251,6 +254,8 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB) sweep_tma_kernel(const __
             const int oh = L::OH + PAD + ((sw - tl0) & 1) + (TS - 1) + lane;
             const int ow = PAD + ((sw - 2 * tl0 - 1) & 1) + 2 * (TS - 1) + lane;
             for (int k = 0; k < nso; ++k, ++q) {
+                // blocks of R steps this stage really has (the last stage is cut at the band's last step)
+                const int nblk = min(TS / R, (t_end - (tbo + k * TS) + R) / R);
                 const int b = q % NBUF;
                 mbar_wait(bar_s + 8u * b, (uint32_t)((q / NBUF) & 1));
                 const double *sb = wbuf + b * L::BUFD;
@@ -261,7 +266,7 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB) sweep_tma_kernel(const __
 #pragma unroll
                 for (int w = 0; w < NW; ++w) xw[w] = pw[w * L::CW];
 #pragma unroll 1
-                for (int blk = 0; blk < TS / R; ++blk) {
+                for (int blk = 0; blk < nblk; ++blk) {
 #pragma unroll
                     for (int u = 0; u < R; ++u) {
                         wa[(R - u) % R] = xa;
@@ -351,6 +356,7 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB) sweep_tma_kernel(const __
             const int oh = L::OH + PAD + ((sw - tl0) & 1) + (TS - 1) + lane;
             const int ow = PAD + ((sw - 2 * tl0) & 1) + 2 * (TS - 1) + lane;
             for (int k = 0; k < nse; ++k, ++q) {
+                const int nblk = min(TS / R, (t_end - (tbe + k * TS) + R) / R);
                 const int b = q % NBUF;
                 mbar_wait(bar_s + 8u * b, (uint32_t)((q / NBUF) & 1));
                 const double *sb = wbuf + b * L::BUFD;
@@ -367,7 +373,7 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB) sweep_tma_kernel(const __
                 }
                 double xu = kA2 ? pu[0] : 0.0;
 #pragma unroll 1
-                for (int blk = 0; blk < TS / R; ++blk) {
+                for (int blk = 0; blk < nblk; ++blk) {
 #pragma unroll
                     for (int u = 0; u < R; ++u) {
                         wa[(R - u) % R] = xa;
@@ -528,11 +534,11 @@ cudaError_t launch_sweep(const SweepParams &P, int mask, int nw, int spin, int t
                           : (P.lmax >= LMAX_LONG ? launch_one<R_TT_LONG, M_TT, 64, 2, false>(P, total_tiles, st)
                                                  : launch_one<R_TT, M_TT, 48, 3, false>(P, total_tiles, st));
         case POL:
-            return banded ? launch_one<R_POL_BAND, POL, 32, 3, false>(P, total_tiles, st)
+            return banded ? launch_one<R_POL_BAND, POL, TJ_TS_BAND, 3, false>(P, total_tiles, st)
                           : (P.lmax >= LMAX_LONG ? launch_one<R_POL, POL, TS_DENSE_LONG, 2, true>(P, total_tiles, st)
                                                         : launch_one<R_POL, POL, TS_DENSE_SHORT, 2, true>(P, total_tiles, st));
         case ALL:
-            return banded ? launch_one<R_POL_BAND, ALL, 32, 3, false>(P, total_tiles, st)
+            return banded ? launch_one<R_POL_BAND, ALL, TJ_TS_BAND, 3, false>(P, total_tiles, st)
                           : (P.lmax >= LMAX_LONG ? launch_one<R_POL, ALL, TS_DENSE_LONG, 2, true>(P, total_tiles, st)
                                                         : launch_one<R_POL, ALL, TS_DENSE_SHORT, 2, true>(P, total_tiles, st));
         default: return cudaErrorInvalidValue;
