@@ -13,6 +13,8 @@ using namespace tj;
 
 namespace {
 
+constexpr int WSET = 7;   // doubles of scratch per window set, in units of nl_alloc: wtt, wtp, wpp, wA (x2), wB (x2)
+
 thread_local char g_errbuf[256] = "CUDA error";
 
 int cuda_fail(cudaError_t e, const char *where)
@@ -75,7 +77,7 @@ struct Call {
     long long N = 0, ld = 0;
     double *TT = nullptr, *TE = nullptr, *ee = nullptr, *EB = nullptr, *bb_copy = nullptr;
     unsigned char *scratch = nullptr;
-    double *wtt = nullptr, *wtp = nullptr, *wpp = nullptr;
+    double *wtt = nullptr, *wtp = nullptr, *wpp = nullptr, *wA = nullptr, *wB = nullptr;
     int *tile_start = nullptr;
 };
 
@@ -431,21 +433,25 @@ int coupling_begin(Call &C, const tj_tables *tables, int lcut, const double *d_W
     C.ntile_w = (int)((C.N + 31) / 32);
 
     // ---- stream-ordered scratch: 3 prefolded windows + tile prefix
-    const size_t wbytes = sizeof(double) * 3 * (size_t)T.nl_alloc * (size_t)nw;
+    // per window set: three plain prefolded arrays + two arrays of pairs (7 nl_alloc doubles)
+    const size_t wbytes = sizeof(double) * WSET * (size_t)T.nl_alloc * (size_t)nw;
     const size_t tbytes = sizeof(int) * (size_t)(C.nb + 1 + 1);
     const size_t tb_al = (tbytes + 15) & ~(size_t)15;
     TJ_CUDA(cudaMallocAsync((void **)&C.scratch, wbytes + tb_al, st), "coupling/scratch");
     C.wtt = (double *)C.scratch + GUARD_LO;
     C.wtp = C.wtt + T.nl_alloc;
     C.wpp = C.wtp + T.nl_alloc;
+    C.wA = C.wpp - GUARD_LO + T.nl_alloc + 2 * GUARD_LO;
+    C.wB = C.wA + 2 * (size_t)T.nl_alloc;
     C.tile_start = (int *)(C.scratch + wbytes);
 
     prof_record(0, st);
     cudaError_t e = cudaSuccess;
     for (int w = 0; w < nw && e == cudaSuccess; ++w) {   // window set w: inputs [w][nW], prefolded arrays 3*nl_alloc apart
-        const size_t wi = (size_t)w * (size_t)nW, wo = (size_t)w * 3 * (size_t)T.nl_alloc;
+        const size_t wi = (size_t)w * (size_t)nW, wo = (size_t)w * WSET * (size_t)T.nl_alloc;
         e = launch_prepare(T, d_Wtt ? d_Wtt + wi : nullptr, d_Wtp ? d_Wtp + wi : nullptr, d_Wpp ? d_Wpp + wi : nullptr,
-                           nW, C.wtt + wo, C.wtp + wo, C.wpp + wo, C.tile_start, C.R, C.l3max_eff, C.banded, st);
+                           nW, C.wtt + wo, C.wtp + wo, C.wpp + wo, C.wA + wo, C.wB + wo, C.tile_start, C.R, C.l3max_eff,
+                           C.banded, st);
     }
     prof_record(1, st);
     if (e == cudaSuccess && C.banded) {
@@ -475,14 +481,14 @@ cudaError_t coupling_sweep(const Call &C, int b0, int b1, cudaStream_t st)
     SweepParams P;
     P.g = T.g; P.ginv = T.ginv; P.h = T.h; P.gA = T.gA; P.gB = T.gB; P.u3 = T.u3;
     P.isd = C.spin == 1 ? T.isu : T.isd;
-    P.wtt = C.wtt; P.wtp = C.wtp; P.wpp = C.wpp;
+    P.wtt = C.wtt; P.wtp = C.wtp; P.wpp = C.wpp; P.wA = C.wA; P.wB = C.wB;
     // a block the instantiated sweep computes but the caller did not ask for has a NULL target and is not stored
     P.TT = C.TT; P.TE = C.TE; P.EE = C.ee; P.EB = C.EB;
     P.tile_start = C.tile_start;
     P.lmax = T.lmax; P.l3max = C.l3max_eff; P.nbands = C.nb; P.lcut = C.banded ? C.lcut : -1; P.ld = C.ld;
     const bool all = (b0 == 0 && b1 == C.nb);
     P.tile_off = all ? 0 : tiles_above(C, b1 - 1);
-    P.wstride = 3 * (long long)T.nl_alloc;
+    P.wstride = WSET * (long long)T.nl_alloc;
     P.ostride = C.N * C.ld;
     const int n = all ? C.ntiles : tiles_above(C, b0 - 1) - P.tile_off;
     return launch_sweep(P, C.mask, C.nw, C.mask == M_TT ? 2 : C.spin, n, st);

@@ -20,7 +20,10 @@ constexpr int GUARD_HI = 768;
 // A thread owns R pairs on ONE anti-diagonal: (l1, l2) = (a+i, c-i), i = 0..R-1, a = band*R.
 // Lanes run along c, so a warp covers rows a..a+R-1 and a skewed window of 32+R-1 columns.
 constexpr int SWEEP_THREADS = 128;   // columns c per CTA
-constexpr int R_POL = 12;           // pairs per thread, fused TT+TE+EE(+EB) sweep, dense storage
+#ifndef TJ_R_POL
+#define TJ_R_POL 12
+#endif
+constexpr int R_POL = TJ_R_POL;           // pairs per thread, fused TT+TE+EE(+EB) sweep, dense storage
 constexpr int R_POL_BAND = 8;       // same, band-limited (short sweeps)
 constexpr int R_TT = 16;            // pairs per thread, TT-only sweep (short or band-limited sweeps)
 constexpr int R_TT_LONG = 32;       // same, dense sweeps at lmax >= LMAX_LONG (measured at lmax = 10^4: 24.9 -> 22.8 ms)
@@ -65,6 +68,7 @@ struct Tables {
 struct SweepParams {
     const double *g, *ginv, *h, *gA, *gB, *u3, *isd;
     const double *wtt, *wtp, *wpp;  // prefolded windows W'_X[l] = (2l+1) W_X[l] / (4 pi), pointer to l = 0
+    const double *wA, *wB;          // the same as pairs: wA[2l..] = (W'_TT, W'_TP)[l], wB[2l..] = (W'_PP, u_l)[l]
     double *TT, *TE, *EE, *EB;      // raw Xi, upper triangle (dense: [l1*ld+l2]; band: [l1*ld + l2-l1+lcut])
     const int *tile_start;          // [nbands+1] exclusive prefix of tiles per band, bands in DESCENDING order
     int lmax, l3max, nbands, lcut;  // lcut < 0: dense storage
@@ -89,8 +93,8 @@ struct WriterParams {
 // kernels / launchers (defined in the .cu files)
 cudaError_t launch_build_tables(const Tables &T, cudaStream_t st);
 cudaError_t launch_prepare(const Tables &T, const double *d_Wtt, const double *d_Wtp, const double *d_Wpp, int nW,
-                           double *wtt, double *wtp, double *wpp, int *tile_start, int R, int l3max_eff, bool banded,
-                           cudaStream_t st);
+                           double *wtt, double *wtp, double *wpp, double *wA, double *wB, int *tile_start, int R,
+                           int l3max_eff, bool banded, cudaStream_t st);
 int sweep_R(int mask, bool banded, int nw, int lmax);   // pairs per thread (= rows per band) of the sweep that serves `mask` for nw window sets
 cudaError_t launch_sweep(const SweepParams &P, int mask, int nw, int spin, int total_tiles, cudaStream_t st);
 cudaError_t launch_writer(const WriterParams &P, cudaStream_t st);

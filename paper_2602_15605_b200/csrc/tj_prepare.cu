@@ -3,6 +3,8 @@
 // a2: W'_X[l] = (2l+1) W_X[l] / (4 pi) for l = 0..nW-1, zero in the guard bands and for l > l3max
 //     (Eq. 3: the (2 j3+1) W~ factor and the 1/(4 pi); the sum simply stops
 //     where the window stops).
+//     The polarised sweeps read the windows as PAIRS, wA[l] = (W'_TT, W'_TP)[l] and wB[l] = (W'_PP, u_l)[l]
+//     (u_l = l(l+1) rides along because the sweep needs it at the same index), written here as well.
 // a3: the upper triangle is cut into row bands of R rows; band `b` needs band_num_tiles(b) CTAs of
 //     SWEEP_THREADS columns.  Work per CTA grows with the band's row index (the sweep has min(l1,l2)+1
 //     steps), so bands are issued in DESCENDING row order: CTA k of the 1-D grid finds its band by a
@@ -18,7 +20,8 @@ constexpr int PREP_THREADS = 256;
 
 __global__ void __launch_bounds__(PREP_THREADS)
 prepare_kernel(const double *__restrict__ Wtt, const double *__restrict__ Wtp, const double *__restrict__ Wpp, int nW,
-               double *wtt, double *wtp, double *wpp, int nl_alloc,
+               double *wtt, double *wtp, double *wpp, double2 *wA, double2 *wB, const double *__restrict__ u3,
+               int nl_alloc,
                int *tile_start, int lmax, int l3max_eff, int R, int banded)
 {
     const double inv4pi = 0.079577471545947667884441881686257181;  // 1/(4 pi)
@@ -29,6 +32,9 @@ prepare_kernel(const double *__restrict__ Wtt, const double *__restrict__ Wtp, c
         if (wtt) wtt[l] = (in && Wtt) ? f * Wtt[l] : 0.0;
         if (wtp) wtp[l] = (in && Wtp) ? f * Wtp[l] : 0.0;
         if (wpp) wpp[l] = (in && Wpp) ? f * Wpp[l] : 0.0;
+        // packed pairs for the polarised sweeps: one 16-byte shared-memory load per pair and step
+        wA[l] = make_double2((in && Wtt) ? f * Wtt[l] : 0.0, (in && Wtp) ? f * Wtp[l] : 0.0);
+        wB[l] = make_double2((in && Wpp) ? f * Wpp[l] : 0.0, u3[l]);
     }
     if (blockIdx.x != 0) return;
 
@@ -57,12 +63,13 @@ prepare_kernel(const double *__restrict__ Wtt, const double *__restrict__ Wtp, c
 }  // namespace
 
 cudaError_t launch_prepare(const Tables &T, const double *d_Wtt, const double *d_Wtp, const double *d_Wpp, int nW,
-                           double *wtt, double *wtp, double *wpp, int *tile_start, int R, int l3max_eff, bool banded,
-                           cudaStream_t st)
+                           double *wtt, double *wtp, double *wpp, double *wA, double *wB, int *tile_start, int R,
+                           int l3max_eff, bool banded, cudaStream_t st)
 {
     int nb = (T.nl_alloc + PREP_THREADS - 1) / PREP_THREADS;
     if (nb > 64) nb = 64;
-    prepare_kernel<<<nb, PREP_THREADS, 0, st>>>(d_Wtt, d_Wtp, d_Wpp, nW, wtt, wtp, wpp, T.nl_alloc, tile_start,
+    prepare_kernel<<<nb, PREP_THREADS, 0, st>>>(d_Wtt, d_Wtp, d_Wpp, nW, wtt, wtp, wpp, (double2 *)wA, (double2 *)wB,
+                                                 T.u3, T.nl_alloc, tile_start,
                                                  T.lmax, l3max_eff, R, banded ? 1 : 0);
     return cudaGetLastError();
 }

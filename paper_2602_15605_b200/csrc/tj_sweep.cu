@@ -54,7 +54,12 @@ namespace {
 // steps per stage of the dense polarised sweep (a multiple of R_POL, even): long stages amortise the stage
 // turn-over (measured at lmax = 10^4: TS = 24 148.8 ms, 48 143.4 ms, 96 141.7 ms) but round every warp's walk
 // up to whole stages, so short sweeps keep the short stage
-constexpr int TS_DENSE_LONG = 96, TS_DENSE_SHORT = 48;
+#ifndef TJ_TS_LONG
+#define TJ_TS_LONG 96
+#define TJ_TS_SHORT 48
+#define TJ_PIPE true
+#endif
+constexpr int TS_DENSE_LONG = TJ_TS_LONG, TS_DENSE_SHORT = TJ_TS_SHORT;
 #ifndef TJ_TS_BAND
 #define TJ_TS_BAND 32
 #endif
@@ -97,10 +102,11 @@ template <int TS, int NW> struct Lay {
     static constexpr int CB = PAD + TS + 32 + 2;       // column ring / h
     static constexpr int CW = PAD + 2 * TS + 32 + 2;   // windows, u3
     static constexpr int OA = 0, OG = OA + CA, OB = OG + CA, OH = OB + CB;
-    static constexpr int OU = OH + CB;
-    // NW window sets (multi-window batching): slot w of TT / TP / PP
-    static constexpr int OW0 = OU + CW, OW1 = OW0 + NW * CW, OW2 = OW1 + NW * CW;
-    static constexpr int BUFD = OW2 + NW * CW;         // doubles per buffer
+    static constexpr int OW0 = OH + CB;                // TT-only sweep: the plain W'_TT slice
+    // polarised sweeps read the windows as pairs (prepare_kernel): (W'_TT, W'_TP)[l] and (W'_PP, u_l)[l], one array
+    // of 2*CW doubles per window set each, in the same region (the TT-only sweep keeps the plain W'_TT slot OW0)
+    static constexpr int OPA = OH + CB, OPB = OPA + NW * 2 * CW;
+    static constexpr int BUFD = OPB + NW * 2 * CW;     // doubles per buffer
 };
 
 // one slice: n doubles starting at table index i0 (any parity) -> buffer offset off (+PAD)
@@ -128,7 +134,9 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB) sweep_tma_kernel(const __
                    kEB = (MASK & M_EB) != 0;
     constexpr bool kEven = kTT || kTE || kEE;
     constexpr bool kA2 = kTE || kEE;
+    constexpr bool kPk = MASK != M_TT;   // windows and u3 come as pairs (wA, wB)
     using L = Lay<TS, NW>;
+    constexpr int NWL = 2 * (TS - 1) + 32;   // l3 values one stage of a warp covers
     static_assert(TS % R == 0 && TS % 2 == 0, "stage length: a multiple of R and even");
 
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -180,33 +188,36 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB) sweep_tma_kernel(const __
         if (q < nso) {
             const int t0 = tbo + q * TS, tl = t0 + TS - 1;
             uint32_t bytes = slice_bytes(a - tl, TS) + slice_bytes(t0, TS) + slice_bytes(cw - R + 1 - tl, TS + 31) +
-                             slice_bytes(sw - tl, TS + 31) + (NW + 1) * slice_bytes(sw - 2 * tl - 1, 2 * (TS - 1) + 32);
+                             slice_bytes(sw - tl, TS + 31) + NW * (2 * NWL * 8);
             mbar_expect_tx(bar, bytes);
             slice(buf, L::OA, P.gA, a - tl, TS, bar);
             slice(buf, L::OG, P.gB, t0, TS, bar);
             slice(buf, L::OB, P.gA, cw - R + 1 - tl, TS + 31, bar);
             slice(buf, L::OH, P.ginv, sw - tl, TS + 31, bar);
 #pragma unroll
-            for (int w = 0; w < NW; ++w)
-                slice(buf, L::OW2 + w * L::CW, P.wpp + w * P.wstride, sw - 2 * tl - 1, 2 * (TS - 1) + 32, bar);
-            slice(buf, L::OU, P.u3, sw - 2 * tl - 1, 2 * (TS - 1) + 32, bar);
+            for (int w = 0; w < NW; ++w)   // pairs (W'_PP, u_l), l = l3lo .. l3lo+NWL-1: always 16-byte aligned
+                bulk_g2s(buf + (uint32_t)(L::OPB + w * 2 * L::CW + 2 * PAD) * 8u,
+                         P.wB + w * P.wstride + 2 * (long long)(sw - 2 * tl - 1), 2 * NWL * 8, bar);
         } else {
             const int t0 = tbe + (q - nso) * TS, tl = t0 + TS - 1;
-            const int nwin = NW * ((kTT ? 1 : 0) + (kTE ? 1 : 0) + (kEE ? 1 : 0)) + (kA2 ? 1 : 0);
             uint32_t bytes = slice_bytes(a - tl, TS) + slice_bytes(t0, TS) + slice_bytes(cw - R + 1 - tl, TS + 31) +
-                             slice_bytes(sw - tl, TS + 31) + nwin * slice_bytes(sw - 2 * tl, 2 * (TS - 1) + 32);
+                             slice_bytes(sw - tl, TS + 31) +
+                             (kPk ? NW * 2 * (2 * NWL * 8) : slice_bytes(sw - 2 * tl, NWL));
             mbar_expect_tx(bar, bytes);
             slice(buf, L::OA, P.g, a - tl, TS, bar);
             slice(buf, L::OG, P.g, t0, TS, bar);
             slice(buf, L::OB, P.g, cw - R + 1 - tl, TS + 31, bar);
             slice(buf, L::OH, P.h, sw - tl, TS + 31, bar);
+            if (kPk) {
 #pragma unroll
-            for (int w = 0; w < NW; ++w) {
-                if (kTT) slice(buf, L::OW0 + w * L::CW, P.wtt + w * P.wstride, sw - 2 * tl, 2 * (TS - 1) + 32, bar);
-                if (kTE) slice(buf, L::OW1 + w * L::CW, P.wtp + w * P.wstride, sw - 2 * tl, 2 * (TS - 1) + 32, bar);
-                if (kEE) slice(buf, L::OW2 + w * L::CW, P.wpp + w * P.wstride, sw - 2 * tl, 2 * (TS - 1) + 32, bar);
+                for (int w = 0; w < NW; ++w) {
+                    const long long o = w * P.wstride + 2 * (long long)(sw - 2 * tl);
+                    bulk_g2s(buf + (uint32_t)(L::OPA + w * 2 * L::CW + 2 * PAD) * 8u, P.wA + o, 2 * NWL * 8, bar);
+                    bulk_g2s(buf + (uint32_t)(L::OPB + w * 2 * L::CW + 2 * PAD) * 8u, P.wB + o, 2 * NWL * 8, bar);
+                }
+            } else {
+                slice(buf, L::OW0, P.wtt, sw - 2 * tl, NWL, bar);
             }
-            if (kA2) slice(buf, L::OU, P.u3, sw - 2 * tl, 2 * (TS - 1) + 32, bar);
         }
     };
     if (lane == 0) {
@@ -252,7 +263,6 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB) sweep_tma_kernel(const __
             const int og = L::OG + PAD + (tbo & 1);
             const int ob = L::OB + PAD + ((cw - R + 1 - tl0) & 1) + (TS - 1) + lane;
             const int oh = L::OH + PAD + ((sw - tl0) & 1) + (TS - 1) + lane;
-            const int ow = PAD + ((sw - 2 * tl0 - 1) & 1) + 2 * (TS - 1) + lane;
             for (int k = 0; k < nso; ++k, ++q) {
                 // blocks of R steps this stage really has (the last stage is cut at the band's last step)
                 const int nblk = min(TS / R, (t_end - (tbo + k * TS) + R) / R);
@@ -260,11 +270,16 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB) sweep_tma_kernel(const __
                 mbar_wait(bar_s + 8u * b, (uint32_t)((q / NBUF) & 1));
                 const double *sb = wbuf + b * L::BUFD;
                 const double *pa = sb + oa, *pg = sb + og, *pb = sb + ob, *ph = sb + oh;
-                const double *pw = sb + L::OW2 + ow, *pu = sb + L::OU + ow;
-                double xa = pa[0], xb = pb[0], xh = ph[0], xg = pg[0], xu = pu[0];
-                double xw[NW];
+                // pairs (W'_PP, u_l) at l3 = s-2t-1: lane's element of step t0+j is 2(TS-1)+lane-2j
+                const double2 *pB = reinterpret_cast<const double2 *>(sb + L::OPB + 2 * PAD) + 2 * (TS - 1) + lane;
+                double xa = pa[0], xb = pb[0], xh = ph[0], xg = pg[0];
+                double xw[NW], xu;
+                {
+                    const double2 v0 = pB[0];
+                    xw[0] = v0.x; xu = v0.y;
 #pragma unroll
-                for (int w = 0; w < NW; ++w) xw[w] = pw[w * L::CW];
+                    for (int w = 1; w < NW; ++w) xw[w] = pB[w * L::CW].x;
+                }
 #pragma unroll 1
                 for (int blk = 0; blk < nblk; ++blk) {
 #pragma unroll
@@ -277,9 +292,12 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB) sweep_tma_kernel(const __
                         for (int w = 0; w < NW; ++w) q3[w] = __dmul_rn(xw[w], hg);
                         const double c3 = xu;
                         xa = pa[-(u + 1)]; xb = pb[-(u + 1)]; xh = ph[-(u + 1)]; xg = pg[u + 1];
+                        {
+                            const double2 v0 = pB[-2 * (u + 1)];
+                            xw[0] = v0.x; xu = v0.y;
 #pragma unroll
-                        for (int w = 0; w < NW; ++w) xw[w] = pw[w * L::CW - 2 * (u + 1)];
-                        xu = pu[-2 * (u + 1)];
+                            for (int w = 1; w < NW; ++w) xw[w] = pB[w * L::CW - 2 * (u + 1)].x;
+                        }
                         double r[R], e[R];
 #pragma unroll
                         for (int i = 0; i < R; ++i) r[i] = __dmul_rn(wa[(i - u + R) % R], wb[(2 * R - i - u) % R]);
@@ -296,7 +314,7 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB) sweep_tma_kernel(const __
 #pragma unroll
                             for (int i = 0; i < R; ++i) acc[w][i] = __fma_rn(r[i], q3[w], acc[w][i]);
                     }
-                    pa -= R; pb -= R; ph -= R; pg += R; pw -= 2 * R; pu -= 2 * R;
+                    pa -= R; pb -= R; ph -= R; pg += R; pB -= 2 * R;
                 }
                 __syncwarp();
                 if (lane == 0 && q + NBUF < ntot) issue(q + NBUF);
@@ -361,17 +379,28 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB) sweep_tma_kernel(const __
                 mbar_wait(bar_s + 8u * b, (uint32_t)((q / NBUF) & 1));
                 const double *sb = wbuf + b * L::BUFD;
                 const double *pa = sb + oa, *pg = sb + og, *pb = sb + ob, *ph = sb + oh;
-                const double *pwtt = sb + L::OW0 + ow, *pwtp = sb + L::OW1 + ow, *pwpp = sb + L::OW2 + ow;
-                const double *pu = sb + L::OU + ow;
+                const double *pwtt = sb + L::OW0 + ow;   // TT-only sweep: plain W'_TT
+                // polarised sweeps: pairs (W'_TT, W'_TP) and (W'_PP, u_l) at l3 = s-2t
+                const double2 *pA = reinterpret_cast<const double2 *>(sb + L::OPA + 2 * PAD) + 2 * (TS - 1) + lane;
+                const double2 *pB = reinterpret_cast<const double2 *>(sb + L::OPB + 2 * PAD) + 2 * (TS - 1) + lane;
                 double xa = pa[0], xb = pb[0], xh = ph[0], xg = pg[0];
-                double xtt[NW], xtp[NW], xpp[NW];
+                double xtt[NW], xtp[NW], xpp[NW], xu = 0.0;
+                // windows (and u3) of the step whose pair element sits `off` pairs from the lane's stage origin
+                auto load_w = [&](int off) {
+                    if (kPk) {
 #pragma unroll
-                for (int w = 0; w < NW; ++w) {
-                    xtt[w] = kTT ? pwtt[w * L::CW] : 0.0;
-                    xtp[w] = kTE ? pwtp[w * L::CW] : 0.0;
-                    xpp[w] = kEE ? pwpp[w * L::CW] : 0.0;
-                }
-                double xu = kA2 ? pu[0] : 0.0;
+                        for (int w = 0; w < NW; ++w) {
+                            const double2 va = pA[w * L::CW + off], vb = pB[w * L::CW + off];
+                            xtt[w] = va.x; xtp[w] = va.y; xpp[w] = vb.x;
+                            if (w == 0) xu = vb.y;
+                        }
+                    } else {
+                        xtt[0] = pwtt[off];
+                    }
+                };
+#pragma unroll
+                for (int w = 0; w < NW; ++w) { xtt[w] = 0.0; xtp[w] = 0.0; xpp[w] = 0.0; }
+                load_w(0);
 #pragma unroll 1
                 for (int blk = 0; blk < nblk; ++blk) {
 #pragma unroll
@@ -388,13 +417,7 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB) sweep_tma_kernel(const __
                         }
                         const double c3 = xu;
                         xa = pa[-(u + 1)]; xb = pb[-(u + 1)]; xh = ph[-(u + 1)]; xg = pg[u + 1];
-#pragma unroll
-                        for (int w = 0; w < NW; ++w) {
-                            if (kTT) xtt[w] = pwtt[w * L::CW - 2 * (u + 1)];
-                            if (kTE) xtp[w] = pwtp[w * L::CW - 2 * (u + 1)];
-                            if (kEE) xpp[w] = pwpp[w * L::CW - 2 * (u + 1)];
-                        }
-                        if (kA2) xu = pu[-2 * (u + 1)];
+                        load_w(-2 * (u + 1));
                         if (PIPE) {
                         // accumulate the PREVIOUS step's products first (their inputs are long ready, so the
                         // 8 FMAs of one window issue back to back and share q through the operand reuse cache)
@@ -449,7 +472,7 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB) sweep_tma_kernel(const __
                         }
                     }
                     pa -= R; pb -= R; ph -= R; pg += R;
-                    pwtt -= 2 * R; pwtp -= 2 * R; pwpp -= 2 * R; pu -= 2 * R;
+                    pwtt -= 2 * R; pA -= 2 * R; pB -= 2 * R;
                 }
                 __syncwarp();
                 if (lane == 0 && q + NBUF < ntot) issue(q + NBUF);
@@ -523,8 +546,8 @@ cudaError_t launch_sweep(const SweepParams &P, int mask, int nw, int spin, int t
     const bool banded = P.lcut >= 0;
     if (spin == 1) {   // dense, one window set; TT-only requests use the spin-independent TT sweep below
         if (banded || nw != 1) return cudaErrorInvalidValue;
-        if (mask == ALL) return launch_one<R_POL, ALL, TS_DENSE_SHORT, 2, true, 1, 1>(P, total_tiles, st);
-        if (mask == POL) return launch_one<R_POL, POL, TS_DENSE_SHORT, 2, true, 1, 1>(P, total_tiles, st);
+        if (mask == ALL) return launch_one<R_POL, ALL, TS_DENSE_SHORT, 2, TJ_PIPE, 1, 1>(P, total_tiles, st);
+        if (mask == POL) return launch_one<R_POL, POL, TS_DENSE_SHORT, 2, TJ_PIPE, 1, 1>(P, total_tiles, st);
     }
     if (nw == 2 && !banded && mask == ALL) return launch_one<R_MULTI2, ALL, 48, 2, true, 2>(P, total_tiles, st);
     if (nw != 1) return cudaErrorInvalidValue;
@@ -535,12 +558,12 @@ cudaError_t launch_sweep(const SweepParams &P, int mask, int nw, int spin, int t
                                                  : launch_one<R_TT, M_TT, 48, 3, false>(P, total_tiles, st));
         case POL:
             return banded ? launch_one<R_POL_BAND, POL, TJ_TS_BAND, 3, false>(P, total_tiles, st)
-                          : (P.lmax >= LMAX_LONG ? launch_one<R_POL, POL, TS_DENSE_LONG, 2, true>(P, total_tiles, st)
-                                                        : launch_one<R_POL, POL, TS_DENSE_SHORT, 2, true>(P, total_tiles, st));
+                          : (P.lmax >= LMAX_LONG ? launch_one<R_POL, POL, TS_DENSE_LONG, 2, TJ_PIPE>(P, total_tiles, st)
+                                                        : launch_one<R_POL, POL, TS_DENSE_SHORT, 2, TJ_PIPE>(P, total_tiles, st));
         case ALL:
             return banded ? launch_one<R_POL_BAND, ALL, TJ_TS_BAND, 3, false>(P, total_tiles, st)
-                          : (P.lmax >= LMAX_LONG ? launch_one<R_POL, ALL, TS_DENSE_LONG, 2, true>(P, total_tiles, st)
-                                                        : launch_one<R_POL, ALL, TS_DENSE_SHORT, 2, true>(P, total_tiles, st));
+                          : (P.lmax >= LMAX_LONG ? launch_one<R_POL, ALL, TS_DENSE_LONG, 2, TJ_PIPE>(P, total_tiles, st)
+                                                        : launch_one<R_POL, ALL, TS_DENSE_SHORT, 2, TJ_PIPE>(P, total_tiles, st));
         default: return cudaErrorInvalidValue;
     }
 }
