@@ -128,7 +128,7 @@ __device__ __forceinline__ int slice_bytes(int i0, int n)
 // "TE" slot accumulates W' X^2 d and the "EE" slot W' X^2 d^2; odd step: (-1 1 0)^2 = Z^2 / (4 u1 u2), so the "EB"
 // slot accumulates W' Z^2; P.isd then holds 1/sqrt(u_l) and the epilogue scales are the same expressions.
 template <int R, int MASK, int TS, int MINB, bool PIPE, int NW, int SPIN>
-__global__ void __launch_bounds__(SWEEP_THREADS, MINB) sweep_tma_kernel(const __grid_constant__ SweepParams P)
+__global__ void __launch_bounds__(SWEEP_THREADS, MINB * (128 / SWEEP_THREADS)) sweep_tma_kernel(const __grid_constant__ SweepParams P)
 {
     constexpr bool kTT = (MASK & M_TT) != 0, kTE = (MASK & M_TE) != 0, kEE = (MASK & M_EE) != 0,
                    kEB = (MASK & M_EB) != 0;
@@ -152,7 +152,7 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB) sweep_tma_kernel(const __
     const int band = P.nbands - 1 - lo;
     const int cb = tile - __ldg(P.tile_start + lo);
     const int a = band * R;
-    const int lane = (int)(threadIdx.x & 31), warp = (int)(threadIdx.x >> 5);
+    const int lane = (int)(threadIdx.x & 31), warp = SWEEP_THREADS == 32 ? 0 : (int)(threadIdx.x >> 5);   // 0: keeps the warp's addresses CTA-uniform
     const int cw = a + cb * SWEEP_THREADS + warp * 32;   // first column of the warp
     const int c = cw + lane;
     const int sw = a + cw;                               // smallest s of the warp
