@@ -489,6 +489,7 @@ cudaError_t coupling_sweep(const Call &C, int b0, int b1, cudaStream_t st)
     const bool all = (b0 == 0 && b1 == C.nb);
     P.tile_off = all ? 0 : tiles_above(C, b1 - 1);
     P.wstride = WSET * (long long)T.nl_alloc;
+    P.even_mask = ~1;
     P.ostride = C.N * C.ld;
     const int n = all ? C.ntiles : tiles_above(C, b0 - 1) - P.tile_off;
     return launch_sweep(P, C.mask, C.nw, C.mask == M_TT ? 2 : C.spin, n, st);

@@ -76,6 +76,7 @@ struct SweepParams {
     double *TT, *TE, *EE, *EB;      // raw Xi, upper triangle (dense: [l1*ld+l2]; band: [l1*ld + l2-l1+lcut])
     const int *tile_start;          // [nbands+1] exclusive prefix of tiles per band, bands in DESCENDING order
     int lmax, l3max, nbands, lcut;  // lcut < 0: dense storage
+    int even_mask;                  // ~1 (see the sweep: keeps a parity out of the compiler's sight)
     int tile_off;                   // first tile of this launch in the descending-band prefix (row-chunked launches)
     long long ld;                   // row stride of the outputs
     long long wstride;              // multi-window: doubles between the prefolded arrays of consecutive window sets

@@ -138,6 +138,7 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB * (128 / SWEEP_THREADS)) s
     using L = Lay<TS, NW>;
     constexpr int NWL = 2 * (TS - 1) + 32;   // l3 values one stage of a warp covers
     static_assert(TS % R == 0 && TS % 2 == 0, "stage length: a multiple of R and even");
+    static_assert(R % 2 == 0, "even R: every block of R steps starts at an even step, which aligns the paired loads of the step factor");
 
     extern __shared__ __align__(128) unsigned char smem_raw[];
     constexpr int NWARP = SWEEP_THREADS / 32;
@@ -173,9 +174,12 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB * (128 / SWEEP_THREADS)) s
     // ---- the warp's walk: odd-J stages first, then even-J stages ----
     const int t_end = a + R - 1;   // last step any pair of the band can have
     int tbo = sw - 1 - P.l3max;    // odd:  l3 = s-2t-1 <= l3max
-    tbo = tbo > 0 ? (tbo + 1) >> 1 : 0;
+    // first steps rounded down to even (an extra step adds exact zeros): the step factor g[t] is then read two steps
+    // per 16-byte load.  The mask is a kernel argument (always ~1) so that the compiler can NOT prove the parity and
+    // pair the row-ring loads too: those go into fixed ring registers and a paired load costs two register moves.
+    tbo = tbo > 0 ? ((tbo + 1) >> 1) & P.even_mask : 0;
     int tbe = sw - P.l3max;        // even: l3 = s-2t   <= l3max
-    tbe = tbe > 0 ? (tbe + 1) >> 1 : 0;
+    tbe = tbe > 0 ? ((tbe + 1) >> 1) & P.even_mask : 0;
     const int nso = (kEB && tbo <= t_end) ? (t_end - tbo + TS) / TS : 0;
     const int nse = (kEven && tbe <= t_end) ? (t_end - tbe + TS) / TS : 0;
     const int ntot = nso + nse;
@@ -272,7 +276,9 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB * (128 / SWEEP_THREADS)) s
                 const double *pa = sb + oa, *pg = sb + og, *pb = sb + ob, *ph = sb + oh;
                 // pairs (W'_PP, u_l) at l3 = s-2t-1: lane's element of step t0+j is 2(TS-1)+lane-2j
                 const double2 *pB = reinterpret_cast<const double2 *>(sb + L::OPB + 2 * PAD) + 2 * (TS - 1) + lane;
-                double xa = pa[0], xb = pb[0], xh = ph[0], xg = pg[0];
+                double xa = pa[0], xb = pb[0], xh = ph[0];
+                double2 xg2 = *reinterpret_cast<const double2 *>(pg);   // g[t] of steps 0, 1
+                double xg = xg2.x;
                 double xw[NW], xu;
                 {
                     const double2 v0 = pB[0];
@@ -291,7 +297,12 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB * (128 / SWEEP_THREADS)) s
 #pragma unroll
                         for (int w = 0; w < NW; ++w) q3[w] = __dmul_rn(xw[w], hg);
                         const double c3 = xu;
-                        xa = pa[-(u + 1)]; xb = pb[-(u + 1)]; xh = ph[-(u + 1)]; xg = pg[u + 1];
+                        xa = pa[-(u + 1)]; xb = pb[-(u + 1)]; xh = ph[-(u + 1)];
+                        // the warp-uniform step factor comes two steps per 16-byte load (the first step is even).  The
+                        // same for the row ring costs more than it saves: its values go into fixed ring registers,
+                        // so half of each pair needs a register move (two instructions) to get there.
+                        if (u % 2 == 0) xg = xg2.y;
+                        else { xg2 = *reinterpret_cast<const double2 *>(pg + (u + 1)); xg = xg2.x; }
                         {
                             const double2 v0 = pB[-2 * (u + 1)];
                             xw[0] = v0.x; xu = v0.y;
@@ -383,7 +394,9 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB * (128 / SWEEP_THREADS)) s
                 // polarised sweeps: pairs (W'_TT, W'_TP) and (W'_PP, u_l) at l3 = s-2t
                 const double2 *pA = reinterpret_cast<const double2 *>(sb + L::OPA + 2 * PAD) + 2 * (TS - 1) + lane;
                 const double2 *pB = reinterpret_cast<const double2 *>(sb + L::OPB + 2 * PAD) + 2 * (TS - 1) + lane;
-                double xa = pa[0], xb = pb[0], xh = ph[0], xg = pg[0];
+                double xa = pa[0], xb = pb[0], xh = ph[0];
+                double2 xg2 = *reinterpret_cast<const double2 *>(pg);   // g[t] of steps 0, 1
+                double xg = xg2.x;
                 double xtt[NW], xtp[NW], xpp[NW], xu = 0.0;
                 // windows (and u3) of the step whose pair element sits `off` pairs from the lane's stage origin
                 auto load_w = [&](int off) {
@@ -416,7 +429,12 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB * (128 / SWEEP_THREADS)) s
                             q2[w] = kEE ? __dmul_rn(xpp[w], hg) : 0.0;
                         }
                         const double c3 = xu;
-                        xa = pa[-(u + 1)]; xb = pb[-(u + 1)]; xh = ph[-(u + 1)]; xg = pg[u + 1];
+                        xa = pa[-(u + 1)]; xb = pb[-(u + 1)]; xh = ph[-(u + 1)];
+                        // the warp-uniform step factor comes two steps per 16-byte load (the first step is even).  The
+                        // same for the row ring costs more than it saves: its values go into fixed ring registers,
+                        // so half of each pair needs a register move (two instructions) to get there.
+                        if (u % 2 == 0) xg = xg2.y;
+                        else { xg2 = *reinterpret_cast<const double2 *>(pg + (u + 1)); xg = xg2.x; }
                         load_w(-2 * (u + 1));
                         if (PIPE) {
                         // accumulate the PREVIOUS step's products first (their inputs are long ready, so the
