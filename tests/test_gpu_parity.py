@@ -536,3 +536,35 @@ def test_literal_eq16_kernel_against_oracle_and_sweep():
     only = binding.coupling_literal(T, None, _t(wl.Wpp), want=("EE",))
     assert torch.equal(only["EE"], lit["EE"])
     T.close()
+
+
+def test_flat_window_closed_form_full_size_lmax10000():
+    """The closed form of the flat window at the HEADLINE size, in the launch configuration bench.py times:
+    W = 1 gives TT = (2 l2+1)/4pi in every one of the 10001^2 entries, TE = 0, EE+EB = (2 l2+1)/4pi on l >= 2
+    (orthogonality of the 3j symbols over l3) -- every (l1,l2,l3) term of the full problem takes part, and no
+    oracle sample is involved.  Also the spin-1 analogue: K11+ + K11- = (2 l2+1)/4pi on l >= 1, K01 = 0."""
+    import torch
+    lmax = 10000
+    N = lmax + 1
+    W = _t(windows.flat(2 * lmax))
+    T = binding.build_tables(lmax)
+    out = binding.coupling_pol(T, W, W, W, want=("TT", "TE", "EE", "EB"))
+    torch.cuda.synchronize()
+    col = ((2.0 * torch.arange(N, dtype=torch.float64, device="cuda") + 1.0) / (4 * math.pi))[None, :]
+    rel_tt = float(((out["TT"] - col).abs() / col).max())
+    s = out["EE"] + out["EB"]
+    rel_s = float(((s - col).abs() / col)[2:, 2:].max())
+    te = float((out["TE"].abs() / col).max())
+    print("flat window lmax=10000: TT rel %.2e, EE+EB rel %.2e, |TE|/scale %.2e" % (rel_tt, rel_s, te))
+    assert rel_tt < 1e-12 and rel_s < 1e-12 and te < 1e-12
+    for k in ("TE", "EE", "EB"):
+        assert torch.all(out[k][:2] == 0) and torch.all(out[k][:, :2] == 0)
+    del out, s
+    sp = binding.coupling_spin1(T, None, W, W, want=("K01", "K11p", "K11m"))
+    torch.cuda.synchronize()
+    s1 = sp["K11p"] + sp["K11m"]
+    rel_1 = float(((s1 - col).abs() / col)[1:, 1:].max())
+    k01 = float((sp["K01"].abs() / col).max())
+    print("spin-1: K11+ + K11- rel %.2e, |K01|/scale %.2e" % (rel_1, k01))
+    assert rel_1 < 1e-12 and k01 < 1e-12
+    T.close()
