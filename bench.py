@@ -283,7 +283,11 @@ def main():
     if nwin > 1:
         # the per-kernel events cover the LAST sweep of the call (one pair of window sets, or a single set when
         # nwin is odd); algorithmic work is counted as for the unbatched method: (8E+5O) per window set
-        last = 2 if nwin % 2 == 0 else 1
+        left, ngroups = nwin, 0
+        while left > 0:        # the library's grouping: threes, a remainder of 4 as 2 + 2, of 2 as one pair
+            last = 2 if left in (2, 4) else 3 if left >= 3 else 1
+            left -= last
+            ngroups += 1
         alg_instr *= last
         alg_flops *= last
     peaks, peak_kind = _peaks()
@@ -295,7 +299,7 @@ def main():
     nmirror = len(blocks) - (1 if "BB" in blocks else 0)
     writer_bytes = int(nmirror * 1.5 * N * width * 8 + (N * width * 8 if "BB" in blocks else 0))
     roofline = {
-        "bound": "alu", "kernel": "sweep_tma_kernel<R=8,TT|TE|EE|EB,TS=48,PIPE,NW=2>" if nwin > 1 and nwin % 2 == 0 else ("sweep_tma_kernel<R=8,TS=32>" if wl.band else "sweep_tma_kernel<R=12,TT|TE|EE|EB,TS=48,PIPE>") if wl.pol else "sweep_tma_kernel<R=16,TT>",
+        "bound": "alu", "kernel": "sweep_tma_kernel<R=6,TT|TE|EE|EB,TS=36,PIPE,NW=3> (last group of the call)" if nwin > 1 else ("sweep_tma_kernel<R=8,TS=32>" if wl.band else "sweep_tma_kernel<R=12,TT|TE|EE|EB,TS=48,PIPE>") if wl.pol else "sweep_tma_kernel<R=16,TT>",
         "achieved": achieved / 1e12, "peak": peak_instr / 1e12, "unit": "T FP64 thread-instr/s",
         "frac": achieved / peak_instr,
         # dram__bytes_read.sum + dram__bytes_write.sum of one sweep launch, from the ncu --set full capture
@@ -367,8 +371,8 @@ def main():
                        "l2": "512 MB flush written between timed steps; each step also writes %.1f GB of output" % (bytes_out / 1e9),
                        "parallelism": "1 problem per GPU" if world > 1 else "single GPU"},
             "roofline": roofline, "cpu_baseline": cpu_baseline, "e2e": e2e, "ablation": ablation,
-            # a batched pair of window sets: 2 prepare + 1 sweep + 2 writer launches; a single set: 3
-            "gpu_launches": ((nwin // 2) * 5 + (nwin % 2) * 3) * args.steps if nwin > 1
+            # per window set one prepare + one writer launch, per group of sets (3, or 2 + 2 for a remainder of 4) one sweep
+            "gpu_launches": (2 * nwin + ngroups) * args.steps if nwin > 1
             else binding.launches_per_call(1) * args.steps,
             "clocks": clocks, "wall_s_timed_region": t_wall, "step_ms": step_ms,
             "context": {"paper_A100_TT_lmax1e4_s": 0.63, "paper_A100_EE_lmax1e4_s": 3.2,

@@ -550,10 +550,11 @@ cudaError_t launch_one(const SweepParams &P, int total_tiles, cudaStream_t st)
 // band-limited sweeps have <= lcut/2+1 steps per pair, so they keep R = 8 and short stages of 32 steps.
 // Multi-window batching (nw window sets in one sweep): the geometric part of a term (r, A2, rA, rAA) is
 // computed once and each window set adds 3 FMAs (1 in the odd branch); the accumulators of nw sets take the
-// registers that R = 12 pairs use otherwise, hence R = 8 for nw = 2 (the only batched instantiation).
+// registers that R = 12 pairs use otherwise, hence R = 8 for nw = 2 and R = 6 for nw = 3.
 int sweep_R(int mask, bool banded, int nw, int lmax)
 {
     if (nw == 2) return R_MULTI2;
+    if (nw == 3) return R_MULTI3;
     if (mask == M_TT) return (!banded && lmax >= LMAX_LONG) ? R_TT_LONG : R_TT;
     return banded ? R_POL_BAND : R_POL;
 }
@@ -568,6 +569,7 @@ cudaError_t launch_sweep(const SweepParams &P, int mask, int nw, int spin, int t
         if (mask == POL) return launch_one<R_POL, POL, TS_DENSE_SHORT, 2, TJ_PIPE, 1, 1>(P, total_tiles, st);
     }
     if (nw == 2 && !banded && mask == ALL) return launch_one<R_MULTI2, ALL, 48, 2, true, 2>(P, total_tiles, st);
+    if (nw == 3 && !banded && mask == ALL) return launch_one<R_MULTI3, ALL, 36, 2, true, 3>(P, total_tiles, st);
     if (nw != 1) return cudaErrorInvalidValue;
     switch (mask) {
         case M_TT:
