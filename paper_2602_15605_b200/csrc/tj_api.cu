@@ -457,11 +457,21 @@ int coupling_begin(Call &C, const tj_tables *tables, int lcut, const double *d_W
     }
     prof_record(1, st);
     if (e == cudaSuccess && C.banded) {
-        // slots of the band whose l2 falls outside 0..lmax (and everything the sweep does not own) are 0
-        const size_t per = (size_t)C.N * (size_t)C.ld * (size_t)nw;
+        // slots of the band whose l2 falls outside 0..lmax are 0: they lie in the first and the last lcut rows, which
+        // are cleared here; every other slot is a valid pair and is written by the sweep (l2 >= l1) or the writer (mirror)
+        const size_t per = (size_t)C.N * (size_t)C.ld;
+        const size_t head = (size_t)(lcut < C.N ? lcut : C.N);           // rows [0, head)
+        const size_t tail0 = (size_t)(C.N - lcut > (long long)head ? C.N - lcut : (long long)head);   // rows [tail0, N)
         double *outs[5] = {d_TT, d_TE, d_EE, d_BB, d_EB};
-        for (int k = 0; k < 5 && e == cudaSuccess; ++k)
-            if (outs[k]) e = cudaMemsetAsync(outs[k], 0, sizeof(double) * per, st);
+        for (int k = 0; k < 5 && e == cudaSuccess; ++k) {
+            if (!outs[k]) continue;
+            for (int w = 0; w < nw && e == cudaSuccess; ++w) {
+                double *m = outs[k] + (size_t)w * per;
+                if (head) e = cudaMemsetAsync(m, 0, sizeof(double) * head * (size_t)C.ld, st);
+                if (e == cudaSuccess && (size_t)C.N > tail0)
+                    e = cudaMemsetAsync(m + tail0 * (size_t)C.ld, 0, sizeof(double) * ((size_t)C.N - tail0) * (size_t)C.ld, st);
+            }
+        }
     }
     if (e != cudaSuccess) { cudaFreeAsync(C.scratch, st); C.scratch = nullptr; return cuda_fail(e, "coupling/prepare"); }
     return TJ_OK;

@@ -233,7 +233,9 @@ def test_band_equals_oracle_and_zero_padded_full(lmax, lcut):
     n = min(lcut + 1, wl.Wtt.size)
     W[:n] = wl.Wtt[:n]
     T = binding.build_tables(lmax)
-    out = binding.coupling_band(T, lcut, _t(W), _t(W), _t(W))
+    # outputs pre-filled with NaN: every slot of the band must be written by the call (values or exact zeros)
+    pre = {k: torch.full((lmax + 1, 2 * lcut + 1), float("nan"), dtype=torch.float64, device="cuda") for k in BLOCKS}
+    out = binding.coupling_band(T, lcut, _t(W), _t(W), _t(W), out=pre)
     torch.cuda.synchronize()
     band = {k: v.cpu().numpy() for k, v in out.items()}
     ref = oracle.coupling_band(lmax, lcut, W, W, W)
@@ -367,8 +369,16 @@ def test_cfg4_band_full_size_sampled():
     wl = windows.config(4)
     lcut = wl.l3max
     T = binding.build_tables(wl.lmax)
-    out = binding.coupling_band(T, lcut, _t(wl.Wtt), _t(wl.Wtp), _t(wl.Wpp))
+    N, width = wl.lmax + 1, 2 * lcut + 1
+    pre = {k: torch.full((N, width), float("nan"), dtype=torch.float64, device="cuda") for k in BLOCKS}
+    out = binding.coupling_band(T, lcut, _t(wl.Wtt), _t(wl.Wtp), _t(wl.Wpp), out=pre)
     torch.cuda.synchronize()
+    # every slot written (outputs were pre-filled with NaN); slots whose l2 is outside 0..lmax exactly 0
+    l2grid = torch.arange(N, device="cuda")[:, None] + torch.arange(-lcut, lcut + 1, device="cuda")[None, :]
+    outside = (l2grid < 0) | (l2grid > wl.lmax)
+    for k in BLOCKS:
+        assert bool(torch.isfinite(out[k]).all()), k
+        assert bool((out[k][outside] == 0).all()), k
     l1, l2 = _sample_pairs(wl.lmax, 3000, 104, band=lcut)
     ref = oracle.coupling_pairs(lcut, wl.Wtt, wl.Wtp, wl.Wpp, l1, l2)
     i1 = torch.as_tensor(l1.astype(np.int64)).cuda()
@@ -390,7 +400,7 @@ def _window_sets(lmax, nwin, seed):
 
 
 def test_multi_window_against_oracle():
-    """3 window sets in one call (one batched pair + one single sweep), each against the oracle."""
+    """3 window sets in one call (one batched sweep of three), each against the oracle."""
     import torch
     lmax, nwin = 150, 3
     Wtt, Wtp, Wpp = _window_sets(lmax, nwin, 100)
