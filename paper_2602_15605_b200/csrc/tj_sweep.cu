@@ -27,21 +27,22 @@
 //     step factor   g [t]               TS          doubles   (broadcast)
 //     column ring   g [cw-R+1+j - t]    TS+31       doubles   (lane j)
 //     1/(J+1)g(p)   h [a+cw+j - t]      TS+31       doubles
-//     windows, u3   W'[a+cw+j - 2t]     2(TS-1)+32  doubles each
+//     windows, u3   pairs (W'_TT, W'_TP)[a+cw+j - 2t] and (W'_PP, u)[a+cw+j - 2t]    2(TS-1)+32 pairs each
+//                   (written as pairs by prepare_kernel; the TT-only sweep reads the plain W'_TT array)
 //
-// (odd-J branch: gA, gB, gA, ginv, W'_PP and u3 at l3 = s-2t-1).  Lane 0 asks the copy engine for the
-// slices of stage k+2 as soon as the warp has finished stage k; the copies land while the warp computes
+// (odd-J branch: gA, gB, gA, ginv and the (W'_PP, u) pairs at l3 = s-2t-1).  Lane 0 asks the copy engine for
+// the slices of stage k+2 as soon as the warp has finished stage k; the copies land while the warp computes
 // stage k+1, and completion is signalled through the buffer's mbarrier (transaction bytes).  The inner
 // loop then reads shared memory only: no L1 miss can stall it, an address is one 32-bit register plus an
-// immediate, and warps stay independent of each other (no CTA barrier; a warp whose columns lie beyond
-// lmax leaves at once, and every warp keeps its own first step for band-limited windows).
+// immediate, and warps are independent of each other -- a CTA is ONE warp (tj_internal.cuh), so that
+// everything the producer computes derives from blockIdx and stays in the uniform datapath.
 //
-// Issue-slot budget (measured): an FP64 instruction takes 2 issue cycles of its SM
-// sub-partition, 3 if it reads three distinct registers none of which the operand reuse cache serves, and
-// every other instruction (LDS, integer) costs about 1.45 cycles of FP64 time.  Hence: as many pairs per
-// thread as registers allow (R = 12 at 2 CTAs/SM for dense sweeps), and, with PIPE, the TE/EE
-// accumulations of step t are issued at the start of step t+1, when all their inputs are ready, so that
-// the R FMAs of one window are adjacent and share q through the reuse cache.
+// Issue model (measured): with the FP64 pipe busy a scheduler issues one warp instruction
+// per ~2 cycles whatever its type, so the time of this kernel is proportional to its instruction count.
+// Hence: as many pairs per thread as registers allow (R = 12 for dense sweeps), 16-byte loads where two
+// values sit side by side (window pairs; the step factor g[t] of two steps), long stages, and, with PIPE,
+// the TE/EE accumulations of step t issued at the start of step t+1, when all their inputs are long ready
+// (measured 0.5 % better than undeferred).
 //
 // Bulk copies need 16-byte aligned source, destination and size; table slices start at any double, so a slice
 // whose first index is odd is fetched from the even index below it and the consumers add that parity `e` to
@@ -52,8 +53,8 @@ namespace tj {
 namespace {
 
 // steps per stage of the dense polarised sweep (a multiple of R_POL, even): long stages amortise the stage
-// turn-over (measured at lmax = 10^4: TS = 24 148.8 ms, 48 143.4 ms, 96 141.7 ms) but round every warp's walk
-// up to whole stages, so short sweeps keep the short stage
+// turn-over (measured at lmax = 10^4 with 4-warp CTAs: TS = 24 148.8 ms, 48 143.4 ms, 96 141.7 ms); short
+// sweeps keep the short stage (less shared memory, finer first/last stage)
 #ifndef TJ_TS_LONG
 #define TJ_TS_LONG 96
 #define TJ_TS_SHORT 48
