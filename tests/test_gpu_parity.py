@@ -578,3 +578,28 @@ def test_flat_window_closed_form_full_size_lmax10000():
     print("spin-1: K11+ + K11- rel %.2e, |K01|/scale %.2e" % (rel_1, k01))
     assert rel_1 < 1e-12 and k01 < 1e-12
     T.close()
+
+
+def test_flat_window_closed_form_beyond_headline_size_lmax16000():
+    """Sizes past the headline config (index arithmetic, guard bands, table range p <= 32001): the flat-window
+    closed form at lmax = 16000, TT-only sweep and fused sweep."""
+    import torch
+    lmax = 16000
+    N = lmax + 1
+    W = _t(windows.flat(2 * lmax))
+    T = binding.build_tables(lmax)
+    col = ((2.0 * torch.arange(N, dtype=torch.float64, device="cuda") + 1.0) / (4 * math.pi))[None, :]
+    TT = binding.coupling_tt(T, W)
+    torch.cuda.synchronize()
+    rel = float(((TT - col).abs() / col).max())
+    assert rel < 1e-12, rel
+    del TT
+    out = binding.coupling_pol(T, None, W, W, want=("TE", "EE", "EB"))
+    torch.cuda.synchronize()
+    s = out["EE"]
+    s += out["EB"]
+    rel_s = float(((s - col).abs() / col)[2:, 2:].max())
+    te = float((out["TE"].abs() / col).max())
+    print("flat window lmax=16000: TT rel %.2e, EE+EB rel %.2e, |TE|/scale %.2e" % (rel, rel_s, te))
+    assert rel_s < 1e-12 and te < 1e-12
+    T.close()
