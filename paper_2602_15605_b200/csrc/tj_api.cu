@@ -571,11 +571,10 @@ int run_literal(const tj_tables *tables, const double *d_Wtt, const double *d_Wp
 // ---- dense call with HOST outputs, pipelined by row chunks ------------------------------------------------
 // Full row l1 of a matrix is final once (i) the sweep and writer of its own row band have run (upper part
 // and diagonal) and (ii) the writers of every band above it have run (they store the mirrored lower part).
-// So the bands are processed in ASCENDING row chunks; after chunk k the rows of chunk k are copied to the
-// host while chunk k+1 is computed.  Successive chunks alternate between two compute streams so that one
+// So the bands are processed in ASCENDING row chunks; after chunk k everything that chunk made final (see the
+// copy loop) is copied to the host while chunk k+1 is computed.  Successive chunks alternate between two compute streams so that one
 // chunk's last CTAs overlap the next chunk's first ones; within a chunk the tiles keep the descending
-// (largest-first) order.  The chunks shrink towards the last rows, where a row is cheap to compute but as
-// large to copy as any other (the exposed tail is the copy of the last chunk).
+// (largest-first) order.
 struct HostPipe {
     cudaStream_t comp[2] = {nullptr, nullptr}, copy = nullptr;
     bool have = false;
@@ -585,7 +584,12 @@ thread_local HostPipe g_pipe;
 int run_coupling_rows_to_host(const tj_tables *tables, const double *d_Wtt, const double *d_Wtp, const double *d_Wpp,
                               int nW, double *const d_out[5], double *const h_out[5], cudaStream_t st)
 {
-    static const double kFrac[] = {0.25, 0.40, 0.50, 0.58, 0.65, 0.71, 0.76, 0.80, 0.84, 0.87, 0.90, 0.925, 0.95, 0.975, 1.0};
+    // chunk ends as fractions of the rows.  The device-to-host link (~35 GB/s measured: 4 GB take ~115 ms against
+    // ~134 ms of compute at lmax = 10^4) must start early and never starve: a first chunk of 20 % of the rows is 10 %
+    // of the work, and with the L-shaped copies below it already releases 36 % of the bytes.  Measured end to end at
+    // config 3: 4 chunks 163 ms, 6 chunks 145 ms, 15 shrinking chunks 137.0 ms, these 10 chunks 135.4 ms
+    // (device-buffer call: 134.4 ms).
+    static const double kFrac[] = {0.20, 0.35, 0.47, 0.57, 0.66, 0.74, 0.81, 0.88, 0.94, 1.0};
     constexpr int KMAX = (int)(sizeof(kFrac) / sizeof(kFrac[0]));
     if (!g_pipe.have) {
         for (int k = 0; k < 2; ++k) TJ_CUDA(cudaStreamCreateWithFlags(&g_pipe.comp[k], cudaStreamNonBlocking), "host pipe");
@@ -626,11 +630,22 @@ int run_coupling_rows_to_host(const tj_tables *tables, const double *d_Wtt, cons
         if (e == cudaSuccess) e = cudaEventRecord(ev[k], cs);
         if (e == cudaSuccess) e = cudaStreamWaitEvent(g_pipe.copy, ev[k], 0);
         if (e == cudaSuccess && k > 0) e = cudaStreamWaitEvent(g_pipe.copy, ev[k - 1], 0);
-        const size_t off = (size_t)r0 * (size_t)C.N, bytes = sizeof(double) * (size_t)(r1 - r0) * (size_t)C.N;
+        // What is final after chunk k: its own rows from column r0 on (their columns < r0 were final earlier), and,
+        // for every row BELOW the chunk, the columns [r0, r1) (the mirror of this chunk's bands).  Copying these two
+        // rectangles per chunk moves every element once and spreads the traffic evenly: the last rows, which are
+        // cheap to compute but as long as any other, have all but their last few columns on the host already.
+        const size_t pitch = sizeof(double) * (size_t)C.N;
         for (int m = 0; m < 5 && e == cudaSuccess; ++m) {
             if (!h_out[m]) continue;
             const double *src = d_out[m] ? d_out[m] : d_out[2];   // BB without its own device matrix: the EE rows
-            e = cudaMemcpyAsync(h_out[m] + off, src + off, bytes, cudaMemcpyDeviceToHost, g_pipe.copy);
+            const size_t o1 = (size_t)r0 * (size_t)C.N + (size_t)r0;
+            e = cudaMemcpy2DAsync(h_out[m] + o1, pitch, src + o1, pitch, sizeof(double) * (size_t)(C.N - r0),
+                                  (size_t)(r1 - r0), cudaMemcpyDeviceToHost, g_pipe.copy);
+            if (e == cudaSuccess && r1 < C.N) {
+                const size_t o2 = (size_t)r1 * (size_t)C.N + (size_t)r0;
+                e = cudaMemcpy2DAsync(h_out[m] + o2, pitch, src + o2, pitch, sizeof(double) * (size_t)(r1 - r0),
+                                      (size_t)(C.N - r1), cudaMemcpyDeviceToHost, g_pipe.copy);
+            }
         }
     }
     // join: the caller's stream continues after everything issued above
