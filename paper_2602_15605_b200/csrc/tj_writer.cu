@@ -3,7 +3,7 @@
 // The sweep leaves Xi(l1,l2), l1 <= l2, in the upper triangle of each output.  Xi is symmetric
 // (PAPER.md:236 as read in DESIGN.md reading #8) and K_{l1 l2} = (2 l2+1) Xi(l1,l2), so
 //     M[l1][l2] = (2 l2+1) Xi,      M[l2][l1] = (2 l1+1) Xi.
-// One CTA owns one 32x32 tile pair (I,J), I <= J: it reads the Xi tile once (coalesced along l2), scales
+// One CTA owns one 32x32 tile pair (I,J), I <= J, of every block: it reads the Xi tile once (coalesced along l2), scales
 // it in place, and writes the mirrored tile through a shared-memory transpose so that both writes are
 // full coalesced row segments.  Both products use the SAME Xi double, so (2 l1+1) M[l1][l2] and
 // (2 l2+1) M[l2][l1] agree to the last rounding.  BB, when requested next to EE, is written from the
@@ -26,44 +26,67 @@ __device__ __forceinline__ long long addr(int r, int c, long long ld, int lcut)
 
 __global__ void __launch_bounds__(WT * WROWS) writer_kernel(const __grid_constant__ WriterParams P)
 {
-    __shared__ double tile[WT][WT + 1];
+    // one CTA handles its tile pair for ALL blocks: every thread has 4 x nmat independent loads in flight before
+    // the first store (the kernel is a latency-bound copy; with one block per CTA it reached 0.70 of the copy peak)
+    __shared__ double tile[4][WT][WT + 1];
     // tile pair decode: blockIdx.x enumerates (I, dJ) with J = I + dJ
     const int I = P.I0 + blockIdx.x / (P.tile_band + 1);
     const int J = I + blockIdx.x % (P.tile_band + 1);
     if (J >= P.ntile) return;
-    const int m = blockIdx.y;
-    double *M = P.M[m];
-    double *bb = (P.bb != nullptr && m == P.bb_src) ? P.bb : nullptr;
     const int tx = threadIdx.x, ty = threadIdx.y;
     const int N = P.lmax + 1;
 
-    // ---- read Xi tile (rows l1 in I, cols l2 in J), scale in place ----
+    // ---- read the Xi tiles (rows l1 in I, cols l2 in J) ----
     const int l2 = J * WT + tx;
+    double xi[4][WT / WROWS];
 #pragma unroll
-    for (int k = 0; k < WT; k += WROWS) {
-        const int l1 = I * WT + ty + k;
-        double xi = 0.0;
-        const bool ok = l1 < N && l2 < N && l2 >= l1 && (P.lcut < 0 || l2 - l1 <= P.lcut);
-        if (ok) {
-            const long long ix = addr(l1, l2, P.ld, P.lcut);
-            xi = M[ix];
-            const double v = xi * (double)(2 * l2 + 1);
-            M[ix] = v;
-            if (bb) bb[ix] = v;
+    for (int m = 0; m < 4; ++m) {
+        if (m >= P.nmat) break;
+        const double *M = P.M[m];
+#pragma unroll
+        for (int k = 0; k < WT; k += WROWS) {
+            const int l1 = I * WT + ty + k;
+            const bool ok = l1 < N && l2 < N && l2 >= l1 && (P.lcut < 0 || l2 - l1 <= P.lcut);
+            xi[m][k / WROWS] = ok ? M[addr(l1, l2, P.ld, P.lcut)] : 0.0;
         }
-        tile[ty + k][tx] = xi;
+    }
+    // ---- scale in place, stage for the transpose ----
+#pragma unroll
+    for (int m = 0; m < 4; ++m) {
+        if (m >= P.nmat) break;
+        double *M = P.M[m];
+        double *bb = (P.bb != nullptr && m == P.bb_src) ? P.bb : nullptr;
+#pragma unroll
+        for (int k = 0; k < WT; k += WROWS) {
+            const int l1 = I * WT + ty + k;
+            const bool ok = l1 < N && l2 < N && l2 >= l1 && (P.lcut < 0 || l2 - l1 <= P.lcut);
+            const double x = xi[m][k / WROWS];
+            if (ok) {
+                const long long ix = addr(l1, l2, P.ld, P.lcut);
+                const double v = x * (double)(2 * l2 + 1);
+                M[ix] = v;
+                if (bb) bb[ix] = v;
+            }
+            tile[m][ty + k][tx] = x;
+        }
     }
     __syncthreads();
-    // ---- mirrored tile: rows r = l2 in J, cols q = l1 in I; strictly lower triangle only ----
+    // ---- mirrored tiles: rows r = l2 in J, cols q = l1 in I; strictly lower triangle only ----
     const int q = I * WT + tx;
 #pragma unroll
-    for (int k = 0; k < WT; k += WROWS) {
-        const int r = J * WT + ty + k;
-        if (r < N && q < N && q < r && (P.lcut < 0 || r - q <= P.lcut)) {
-            const double v = tile[tx][ty + k] * (double)(2 * q + 1);
-            const long long ix = addr(r, q, P.ld, P.lcut);
-            M[ix] = v;
-            if (bb) bb[ix] = v;
+    for (int m = 0; m < 4; ++m) {
+        if (m >= P.nmat) break;
+        double *M = P.M[m];
+        double *bb = (P.bb != nullptr && m == P.bb_src) ? P.bb : nullptr;
+#pragma unroll
+        for (int k = 0; k < WT; k += WROWS) {
+            const int r = J * WT + ty + k;
+            if (r < N && q < N && q < r && (P.lcut < 0 || r - q <= P.lcut)) {
+                const double v = tile[m][tx][ty + k] * (double)(2 * q + 1);
+                const long long ix = addr(r, q, P.ld, P.lcut);
+                M[ix] = v;
+                if (bb) bb[ix] = v;
+            }
         }
     }
 }
@@ -73,7 +96,7 @@ __global__ void __launch_bounds__(WT * WROWS) writer_kernel(const __grid_constan
 cudaError_t launch_writer(const WriterParams &P, cudaStream_t st)
 {
     if (P.nmat <= 0 || P.I1 <= P.I0) return cudaSuccess;
-    dim3 grid((unsigned)((P.I1 - P.I0) * (P.tile_band + 1)), (unsigned)P.nmat, 1);
+    dim3 grid((unsigned)((P.I1 - P.I0) * (P.tile_band + 1)), 1, 1);
     dim3 block(WT, WROWS, 1);
     writer_kernel<<<grid, block, 0, st>>>(P);
     return cudaGetLastError();
