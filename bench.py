@@ -304,7 +304,7 @@ def main():
         "frac": achieved / peak_instr,
         # dram__bytes_read.sum + dram__bytes_write.sum of one sweep launch, from the ncu --set full capture
         # profiles/r1_ncu_full_cfg3.md (config 3 only; other configs: not captured)
-        "traffic": 1.573e9 if (args.config == 3 and wl.pol) else None,
+        "traffic": 1.571e9 if (args.config == 3 and wl.pol) else None,
         "peak_source": "derived: %d SMs x %d FP64 lanes/clk x %.0f MHz (DESIGN.md 6; MEASURED_PEAKS.json has no FP64 entry)"
                        % (SM_COUNT, FP64_LANES_PER_SM, sm_max),
         "algorithmic_instr_per_launch": alg_instr, "algorithmic_flops_per_launch": alg_flops,
