@@ -533,12 +533,10 @@ cudaError_t launch_one(const SweepParams &P, int total_tiles, cudaStream_t st)
     if (total_tiles <= 0) return cudaSuccess;
     constexpr int NWARP = SWEEP_THREADS / 32;
     constexpr size_t smem = (size_t)NWARP * NBUF * Lay<TS, NW>::BUFD * 8 + (size_t)NWARP * NBUF * 8;
-    static bool attr_set = false;   // per instantiation
-    if (!attr_set) {
+    if (smem > 48 * 1024) {   // opt-in beyond the default limit (per device, so not cached; one-warp CTAs stay below it)
         cudaError_t e = cudaFuncSetAttribute(sweep_tma_kernel<R, MASK, TS, MINB, PIPE, NW, SPIN>,
                                              cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
-        attr_set = true;
     }
     sweep_tma_kernel<R, MASK, TS, MINB, PIPE, NW, SPIN><<<total_tiles, SWEEP_THREADS, smem, st>>>(P);
     return cudaGetLastError();
