@@ -99,7 +99,7 @@ int tj_coupling_band(const tj_tables *tables, int lcut,
  * (same arithmetic per entry, so they agree to the last bit).
  *   Windows: [nwin][nW] row-major, nW = l3max+1.  Outputs: [nwin][(lmax+1)^2].  NULL rules as tj_coupling_pol;
  *   requests for all of TT, TE, EE (or BB) and EB run three sets per sweep (a remainder of two or four sets: two per
- *   sweep), other requests one set per sweep.
+ *   sweep), requests for TT alone four windows per sweep (then two, then one), other requests one set per sweep.
  */
 int tj_coupling_multi(const tj_tables *tables, int nwin,
                       const double *d_Wtt, const double *d_Wtp, const double *d_Wpp, int nW,

@@ -215,11 +215,14 @@ int tj_coupling_multi(const tj_tables *tables, int nwin, const double *d_Wtt, co
     const size_t per = ((size_t)tables->T.lmax + 1) * ((size_t)tables->T.lmax + 1);
     // the batched sweep is instantiated for the full set of blocks; any other request runs one window set at a time
     const bool full = d_Wtt && d_Wtp && d_Wpp && d_TT && d_TE && (d_EE || d_BB) && d_EB;
+    // TT alone (many temperature map pairs, covariance windows): four windows per sweep, then two, then one
+    const bool tt_only = d_Wtt && d_TT && !d_TE && !d_EE && !d_BB && !d_EB;
     int w = 0;
     while (w < nwin) {
         // groups of three window sets per sweep; a remainder of 4 goes as 2 + 2, of 2 as one pair
         const int left = nwin - w;
-        const int nw = !full ? 1 : (left == 4 || left == 2) ? 2 : left >= 3 ? 3 : 1;
+        const int nw = tt_only ? (left >= 4 ? 4 : left >= 2 ? 2 : 1)
+                               : !full ? 1 : (left == 4 || left == 2) ? 2 : left >= 3 ? 3 : 1;
         const size_t wi = (size_t)w * (size_t)nW, oi = (size_t)w * per;
         int rc = run_coupling(tables, -1, d_Wtt ? d_Wtt + wi : nullptr, d_Wtp ? d_Wtp + wi : nullptr,
                               d_Wpp ? d_Wpp + wi : nullptr, nW, d_TT ? d_TT + oi : nullptr, d_TE ? d_TE + oi : nullptr,

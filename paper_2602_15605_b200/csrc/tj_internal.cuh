@@ -34,6 +34,7 @@ constexpr int R_TT_LONG = 32;       // same, dense sweeps at lmax >= LMAX_LONG (
 constexpr int LMAX_LONG = 4096;     // from here on a dense sweep uses the long-sweep geometry (R_TT_LONG; 96-step stages)
 constexpr int R_MULTI2 = 8;         // pairs per thread, 2 window sets per sweep (tj_coupling_multi)
 constexpr int R_MULTI3 = 6;         // pairs per thread, 3 window sets per sweep
+constexpr int R_TT_MULTI = 16;      // pairs per thread, TT-only sweep of 2 or 4 windows
 
 // mask bits of the blocks one sweep computes
 constexpr int M_TT = 1, M_TE = 2, M_EE = 4, M_EB = 8;

@@ -98,16 +98,16 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t
 }
 
 // capacities (doubles, all even) of the slices inside one stage buffer
-template <int TS, int NW> struct Lay {
+template <int TS, int NW, bool PK> struct Lay {
     static constexpr int CA = PAD + TS + 2;            // row ring / step factor
     static constexpr int CB = PAD + TS + 32 + 2;       // column ring / h
     static constexpr int CW = PAD + 2 * TS + 32 + 2;   // windows, u3
     static constexpr int OA = 0, OG = OA + CA, OB = OG + CA, OH = OB + CB;
-    static constexpr int OW0 = OH + CB;                // TT-only sweep: the plain W'_TT slice
+    static constexpr int OW0 = OH + CB;                // TT-only sweep: the plain W'_TT slices, one per window set
     // polarised sweeps read the windows as pairs (prepare_kernel): (W'_TT, W'_TP)[l] and (W'_PP, u_l)[l], one array
     // of 2*CW doubles per window set each, in the same region (the TT-only sweep keeps the plain W'_TT slot OW0)
     static constexpr int OPA = OH + CB, OPB = OPA + NW * 2 * CW;
-    static constexpr int BUFD = OPB + NW * 2 * CW;     // doubles per buffer
+    static constexpr int BUFD = PK ? OPB + NW * 2 * CW : OW0 + NW * CW;   // doubles per buffer
 };
 
 // one slice: n doubles starting at table index i0 (any parity) -> buffer offset off (+PAD)
@@ -136,7 +136,7 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB * (128 / SWEEP_THREADS)) s
     constexpr bool kEven = kTT || kTE || kEE;
     constexpr bool kA2 = kTE || kEE;
     constexpr bool kPk = MASK != M_TT;   // windows and u3 come as pairs (wA, wB)
-    using L = Lay<TS, NW>;
+    using L = Lay<TS, NW, kPk>;
     constexpr int NWL = 2 * (TS - 1) + 32;   // l3 values one stage of a warp covers
     static_assert(TS % R == 0 && TS % 2 == 0, "stage length: a multiple of R and even");
     static_assert(R % 2 == 0, "even R: every block of R steps starts at an even step, which aligns the paired loads of the step factor");
@@ -207,7 +207,7 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB * (128 / SWEEP_THREADS)) s
             const int t0 = tbe + (q - nso) * TS, tl = t0 + TS - 1;
             uint32_t bytes = slice_bytes(a - tl, TS) + slice_bytes(t0, TS) + slice_bytes(cw - R + 1 - tl, TS + 31) +
                              slice_bytes(sw - tl, TS + 31) +
-                             (kPk ? NW * 2 * (2 * NWL * 8) : slice_bytes(sw - 2 * tl, NWL));
+                             (kPk ? NW * 2 * (2 * NWL * 8) : NW * slice_bytes(sw - 2 * tl, NWL));
             mbar_expect_tx(bar, bytes);
             slice(buf, L::OA, P.g, a - tl, TS, bar);
             slice(buf, L::OG, P.g, t0, TS, bar);
@@ -221,7 +221,9 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB * (128 / SWEEP_THREADS)) s
                     bulk_g2s(buf + (uint32_t)(L::OPB + w * 2 * L::CW + 2 * PAD) * 8u, P.wB + o, 2 * NWL * 8, bar);
                 }
             } else {
-                slice(buf, L::OW0, P.wtt, sw - 2 * tl, NWL, bar);
+#pragma unroll
+                for (int w = 0; w < NW; ++w)
+                    slice(buf, L::OW0 + w * L::CW, P.wtt + w * P.wstride, sw - 2 * tl, NWL, bar);
             }
         }
     };
@@ -409,7 +411,8 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB * (128 / SWEEP_THREADS)) s
                             if (w == 0) xu = vb.y;
                         }
                     } else {
-                        xtt[0] = pwtt[off];
+#pragma unroll
+                        for (int w = 0; w < NW; ++w) xtt[w] = pwtt[w * L::CW + off];
                     }
                 };
 #pragma unroll
@@ -532,7 +535,7 @@ cudaError_t launch_one(const SweepParams &P, int total_tiles, cudaStream_t st)
 {
     if (total_tiles <= 0) return cudaSuccess;
     constexpr int NWARP = SWEEP_THREADS / 32;
-    constexpr size_t smem = (size_t)NWARP * NBUF * Lay<TS, NW>::BUFD * 8 + (size_t)NWARP * NBUF * 8;
+    constexpr size_t smem = (size_t)NWARP * NBUF * Lay<TS, NW, MASK != M_TT>::BUFD * 8 + (size_t)NWARP * NBUF * 8;
     if (smem > 48 * 1024) {   // opt-in beyond the default limit (per device, so not cached; one-warp CTAs stay below it)
         cudaError_t e = cudaFuncSetAttribute(sweep_tma_kernel<R, MASK, TS, MINB, PIPE, NW, SPIN>,
                                              cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -552,6 +555,7 @@ cudaError_t launch_one(const SweepParams &P, int total_tiles, cudaStream_t st)
 // registers that R = 12 pairs use otherwise, hence R = 8 for nw = 2 and R = 6 for nw = 3.
 int sweep_R(int mask, bool banded, int nw, int lmax)
 {
+    if (mask == M_TT && nw > 1) return R_TT_MULTI;
     if (nw == 2) return R_MULTI2;
     if (nw == 3) return R_MULTI3;
     if (mask == M_TT) return (!banded && lmax >= LMAX_LONG) ? R_TT_LONG : R_TT;
@@ -569,6 +573,8 @@ cudaError_t launch_sweep(const SweepParams &P, int mask, int nw, int spin, int t
     }
     if (nw == 2 && !banded && mask == ALL) return launch_one<R_MULTI2, ALL, 48, 2, true, 2>(P, total_tiles, st);
     if (nw == 3 && !banded && mask == ALL) return launch_one<R_MULTI3, ALL, 36, 2, true, 3>(P, total_tiles, st);
+    if (nw == 4 && !banded && mask == M_TT) return launch_one<R_TT_MULTI, M_TT, 48, 2, false, 4>(P, total_tiles, st);
+    if (nw == 2 && !banded && mask == M_TT) return launch_one<R_TT_MULTI, M_TT, 48, 2, false, 2>(P, total_tiles, st);
     if (nw != 1) return cudaErrorInvalidValue;
     switch (mask) {
         case M_TT:

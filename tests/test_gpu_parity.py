@@ -603,3 +603,28 @@ def test_flat_window_closed_form_beyond_headline_size_lmax16000():
     print("flat window lmax=16000: TT rel %.2e, EE+EB rel %.2e, |TE|/scale %.2e" % (rel, rel_s, te))
     assert rel_s < 1e-12 and te < 1e-12
     T.close()
+
+
+def test_multi_window_tt_only_bitwise_and_oracle():
+    """TT alone for 7 windows (sweeps of 4 + 2 + 1 windows): bitwise equal to tj_coupling_tt per window, and
+    against the oracle at a small size."""
+    import torch
+    lmax, nwin = 900, 7
+    Wtt, _, _ = _window_sets(lmax, nwin, 300)
+    T = binding.build_tables(lmax)
+    out = binding.coupling_multi(T, _t(Wtt), None, None, want=("TT",))
+    torch.cuda.synchronize()
+    for w in range(nwin):
+        one = binding.coupling_tt(T, _t(Wtt[w]))
+        torch.cuda.synchronize()
+        assert torch.equal(out["TT"][w], one), w
+    T.close()
+    lmax = 130
+    Wtt, _, _ = _window_sets(lmax, 4, 310)
+    T = binding.build_tables(lmax)
+    out = binding.coupling_multi(T, _t(Wtt), None, None, want=("TT",))
+    torch.cuda.synchronize()
+    for w in range(4):
+        ref = oracle.coupling_full(lmax, 2 * lmax, Wtt[w], None, None)["TT"]
+        assert_parity(out["TT"][w].cpu().numpy(), ref, "multi TT set %d" % w)
+    T.close()
