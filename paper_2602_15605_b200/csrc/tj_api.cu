@@ -575,9 +575,9 @@ int run_literal(const tj_tables *tables, const double *d_Wtt, const double *d_Wp
 // Full row l1 of a matrix is final once (i) the sweep and writer of its own row band have run (upper part
 // and diagonal) and (ii) the writers of every band above it have run (they store the mirrored lower part).
 // So the bands are processed in ASCENDING row chunks; after chunk k everything that chunk made final (see the
-// copy loop) is copied to the host while chunk k+1 is computed.  Successive chunks alternate between two compute streams so that one
-// chunk's last CTAs overlap the next chunk's first ones; within a chunk the tiles keep the descending
-// (largest-first) order.
+// copy loop) is copied to the host while chunk k+1 is computed.  Successive chunks alternate between two compute
+// streams so that one chunk's last CTAs overlap the next chunk's first ones; within a chunk the tiles keep the
+// descending (largest-first) order.
 struct HostPipe {
     cudaStream_t comp[2] = {nullptr, nullptr}, copy = nullptr;
     bool have = false;
@@ -587,8 +587,9 @@ thread_local HostPipe g_pipe;
 int run_coupling_rows_to_host(const tj_tables *tables, const double *d_Wtt, const double *d_Wtp, const double *d_Wpp,
                               int nW, double *const d_out[5], double *const h_out[5], cudaStream_t st)
 {
-    // chunk ends as fractions of the rows.  The device-to-host link (~35 GB/s measured: 4 GB take ~115 ms against
-    // ~134 ms of compute at lmax = 10^4) must start early and never starve: a first chunk of 20 % of the rows is 10 %
+    // chunk ends as fractions of the rows.  The device-to-host copies (rectangles with a row pitch: an effective
+    // ~35 GB/s here, where one contiguous copy reaches 54 GB/s, so 4 GB take ~115 ms against ~134 ms of compute at
+    // lmax = 10^4) must start early and never starve: a first chunk of 20 % of the rows is 10 %
     // of the work, and with the L-shaped copies below it already releases 36 % of the bytes.  Measured end to end at
     // config 3: 4 chunks 163 ms, 6 chunks 145 ms, 15 shrinking chunks 137.0 ms, these 10 chunks 135.4 ms
     // (device-buffer call: 134.4 ms).
