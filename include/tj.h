@@ -124,6 +124,22 @@ int tj_coupling_spin1(const tj_tables *tables,
                       void *cuda_stream);
 
 /*
+ * tj_coupling_rows -- the full rows row_lo <= l1 < row_hi of the matrices tj_coupling_pol would give, in compact
+ * storage: out[(l1-row_lo)*(lmax+1) + l2] = K_{l1 l2}, all columns l2 = 0..lmax.
+ * Every (l1,l2) is independent, so a matrix can be cut into row blocks that are computed
+ * anywhere -- one block per GPU with no exchange, or block after block when the whole matrix is not wanted at
+ * once.  Entries left of the diagonal are obtained through the symmetry of Xi, so a block costs its
+ * own upper-triangle rows plus the pairs (l1 < row_lo, l2 in the block); values are bit-identical to the rows of
+ * the full call.  0 <= row_lo < row_hi <= lmax+1; windows, NULL rules and BB as tj_coupling_pol; each output holds
+ * (row_hi-row_lo)*(lmax+1) doubles.
+ */
+int tj_coupling_rows(const tj_tables *tables,
+                     const double *d_Wtt, const double *d_Wtp, const double *d_Wpp, int nW,
+                     int row_lo, int row_hi,
+                     double *d_TT, double *d_TE, double *d_EE, double *d_BB, double *d_EB,
+                     void *cuda_stream);
+
+/*
  * tj_coupling_literal -- ABLATION, not the hot path: the paper's own evaluation restated as
  * one plain kernel -- one thread per (l1,l2) of the upper triangle, serial l3 loop in steps of 2 with direct
  * table lookups, K^{TT} from Eq. 10 and K^{EE} from Eq. 16

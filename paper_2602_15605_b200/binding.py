@@ -18,7 +18,7 @@ TJ_OK, TJ_EINVAL, TJ_ENOMEM, TJ_ECUDA = 0, -1, -2, -3
 # every symbol include/tj.h declares (tests/test_abi.py checks the header against this and the .so)
 SYMBOLS = (
     "tj_build_tables", "tj_free_tables", "tj_tables_info", "tj_tables_copy",
-    "tj_coupling_tt", "tj_coupling_pol", "tj_coupling_band", "tj_coupling_multi", "tj_coupling_spin1", "tj_coupling_literal", "tj_coupling_host",
+    "tj_coupling_tt", "tj_coupling_pol", "tj_coupling_band", "tj_coupling_multi", "tj_coupling_spin1", "tj_coupling_rows", "tj_coupling_literal", "tj_coupling_host",
     "tj_l3_range", "tj_sweep_counts", "tj_fp64_probe", "tj_profile_enable", "tj_profile_get",
     "tj_launches_per_call", "tj_strerror",
 )
@@ -54,6 +54,7 @@ def load_library() -> ctypes.CDLL:
     L.tj_coupling_band.argtypes = [vp, ci, vp, vp, vp, vp, vp, vp, vp, vp, vp]
     L.tj_coupling_multi.argtypes = [vp, ci, vp, vp, vp, ci, vp, vp, vp, vp, vp, vp]
     L.tj_coupling_spin1.argtypes = [vp, vp, vp, vp, ci, vp, vp, vp, vp, vp]
+    L.tj_coupling_rows.argtypes = [vp, vp, vp, vp, ci, ci, ci, vp, vp, vp, vp, vp, vp]
     L.tj_coupling_literal.argtypes = [vp, vp, vp, ci, vp, vp, vp]
     L.tj_coupling_host.argtypes = [vp, ci, ci, vp, vp, vp, vp, vp, vp, vp, vp, vp]
     L.tj_l3_range.argtypes = [ci, ci, ci, ci, ip, ip, ip]
@@ -237,6 +238,24 @@ def coupling_spin1(tables: Tables, W00, W01, W11, want=_SPIN1, out=None, stream=
     _check(load_library().tj_coupling_spin1(tables.handle, _dev_ptr(W00, nW, "W00"), _dev_ptr(W01, nW, "W01"),
                                             _dev_ptr(W11, nW, "W11"), nW, *args, _stream_ptr(stream)),
            "tj_coupling_spin1")
+    return {k: out[k] for k in want}
+
+
+def coupling_rows(tables: Tables, Wtt, Wtp, Wpp, row_lo: int, row_hi: int, want=_BLOCKS, out=None, stream=None):
+    """tj_coupling_rows: rows row_lo..row_hi-1 of every block in `want`, each [(row_hi-row_lo), (lmax+1)]."""
+    import torch
+    N = tables.lmax + 1
+    nW = tables.l3max + 1
+    nr = int(row_hi) - int(row_lo)
+    dev = next(w for w in (Wtt, Wtp, Wpp) if w is not None).device
+    out = {} if out is None else dict(out)
+    for k in want:
+        if k not in out:
+            out[k] = torch.empty((nr, N), dtype=torch.float64, device=dev)
+    args = [_dev_ptr(out.get(k) if k in want else None, nr * N, k) for k in _BLOCKS]
+    _check(load_library().tj_coupling_rows(tables.handle, _dev_ptr(Wtt, nW, "Wtt"), _dev_ptr(Wtp, nW, "Wtp"),
+                                           _dev_ptr(Wpp, nW, "Wpp"), nW, int(row_lo), int(row_hi), *args,
+                                           _stream_ptr(stream)), "tj_coupling_rows")
     return {k: out[k] for k in want}
 
 

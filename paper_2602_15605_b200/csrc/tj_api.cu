@@ -58,11 +58,11 @@ void prof_record(int i, cudaStream_t st)
     if (i == 4) g_prof.valid = true;
 }
 
-int total_tiles(int lmax, int l3max, int R, bool banded)
+int total_tiles(int lmax, int l3max, int R, bool banded, int row_lo, int row_hi)
 {
     long long n = 0;
     const int nb = num_bands(lmax, R);
-    for (int b = 0; b < nb; ++b) n += band_num_tiles(lmax, l3max, R, b, banded);
+    for (int b = 0; b < nb; ++b) n += band_num_tiles(lmax, l3max, R, b, banded, row_lo, row_hi);
     return n > 0x7fffffffLL ? -1 : (int)n;
 }
 
@@ -74,6 +74,8 @@ struct Call {
     int nw = 1;                     // window sets per sweep (tj_coupling_multi: 2)
     int spin = 2;                   // 2: TT/TE/EE/EB; 1: K00/K01/K11+/K11- in the same slots (tj_coupling_spin1)
     int nW = 0;                     // entries per window
+    int row_lo = 0, row_hi = 0;     // full rows [row_lo, row_hi) are computed (tj_coupling_rows; else 0, lmax+1)
+    bool rows = false;              // row-block outputs
     long long N = 0, ld = 0;
     double *TT = nullptr, *TE = nullptr, *ee = nullptr, *EB = nullptr, *bb_copy = nullptr;
     unsigned char *scratch = nullptr;
@@ -85,6 +87,8 @@ struct Call {
 int run_coupling(const tj_tables *tables, int lcut, const double *d_Wtt, const double *d_Wtp, const double *d_Wpp,
                  int nW, double *d_TT, double *d_TE, double *d_EE, double *d_BB, double *d_EB, cudaStream_t st, int nw = 1,
                  int spin = 2);
+int run_rows(const tj_tables *tables, const double *d_Wtt, const double *d_Wtp, const double *d_Wpp, int nW, int row_lo,
+             int row_hi, double *d_TT, double *d_TE, double *d_EE, double *d_BB, double *d_EB, cudaStream_t st);
 int run_coupling_rows_to_host(const tj_tables *tables, const double *d_Wtt, const double *d_Wtp, const double *d_Wpp,
                               int nW, double *const d_out[5], double *const h_out[5], cudaStream_t st);
 int run_literal(const tj_tables *tables, const double *d_Wtt, const double *d_Wpp, int nW, double *d_TT, double *d_EE,
@@ -241,6 +245,16 @@ int tj_coupling_spin1(const tj_tables *tables, const double *d_W00, const double
     // same sweep, spin-1 algebra: K00 rides in the TT slot, K01 in TE, K11+ in EE, K11- in EB
     return run_coupling(tables, -1, d_W00, d_W01, d_W11, nW, d_K00, d_K01, d_K11p, nullptr, d_K11m,
                         (cudaStream_t)cuda_stream, 1, 1);
+}
+
+int tj_coupling_rows(const tj_tables *tables, const double *d_Wtt, const double *d_Wtp, const double *d_Wpp, int nW,
+                     int row_lo, int row_hi, double *d_TT, double *d_TE, double *d_EE, double *d_BB, double *d_EB,
+                     void *cuda_stream)
+{
+    if (!tables) return TJ_EINVAL;
+    if (nW != tables->T.l3max + 1) return TJ_EINVAL;
+    if (row_lo < 0 || row_hi <= row_lo || row_hi > tables->T.lmax + 1) return TJ_EINVAL;
+    return run_rows(tables, d_Wtt, d_Wtp, d_Wpp, nW, row_lo, row_hi, d_TT, d_TE, d_EE, d_BB, d_EB, (cudaStream_t)cuda_stream);
 }
 
 int tj_coupling_literal(const tj_tables *tables, const double *d_Wtt, const double *d_Wpp, int nW, double *d_TT,
@@ -408,7 +422,7 @@ namespace {
 // ---- one coupling call, in pieces (the host-buffer path launches the middle two per row chunk) -------------
 int coupling_begin(Call &C, const tj_tables *tables, int lcut, const double *d_Wtt, const double *d_Wtp,
                    const double *d_Wpp, int nW, double *d_TT, double *d_TE, double *d_EE, double *d_BB, double *d_EB,
-                   cudaStream_t st, int nw = 1, int spin = 2)
+                   cudaStream_t st, int nw = 1, int spin = 2, int row_lo = -1, int row_hi = -1)
 {
     const Tables &T = tables->T;
     C.T = &T;
@@ -431,8 +445,11 @@ int coupling_begin(Call &C, const tj_tables *tables, int lcut, const double *d_W
     C.R = sweep_R(C.mask, C.banded, nw, T.lmax);
     C.l3max_eff = C.banded ? lcut : T.l3max;
     C.N = (long long)T.lmax + 1;
+    C.rows = row_lo >= 0;
+    C.row_lo = C.rows ? row_lo : 0;
+    C.row_hi = C.rows ? row_hi : T.lmax + 1;
     C.ld = C.banded ? (long long)(2 * lcut + 1) : C.N;
-    C.ntiles = total_tiles(T.lmax, C.l3max_eff, C.R, C.banded);
+    C.ntiles = total_tiles(T.lmax, C.l3max_eff, C.R, C.banded, C.row_lo, C.row_hi);
     if (C.ntiles < 0) return TJ_EINVAL;
     C.nb = num_bands(T.lmax, C.R);
     C.ntile_w = (int)((C.N + 31) / 32);
@@ -456,7 +473,7 @@ int coupling_begin(Call &C, const tj_tables *tables, int lcut, const double *d_W
         const size_t wi = (size_t)w * (size_t)nW, wo = (size_t)w * WSET * (size_t)T.nl_alloc;
         e = launch_prepare(T, d_Wtt ? d_Wtt + wi : nullptr, d_Wtp ? d_Wtp + wi : nullptr, d_Wpp ? d_Wpp + wi : nullptr,
                            nW, C.wtt + wo, C.wtp + wo, C.wpp + wo, C.wA + wo, C.wB + wo, C.tile_start, C.R, C.l3max_eff,
-                           C.banded, st);
+                           C.banded, C.row_lo, C.row_hi, st);
     }
     prof_record(1, st);
     if (e == cudaSuccess && C.banded) {
@@ -485,7 +502,7 @@ int coupling_begin(Call &C, const tj_tables *tables, int lcut, const double *d_W
 int tiles_above(const Call &C, int b)
 {
     long long n = 0;
-    for (int k = C.nb - 1; k > b; --k) n += band_num_tiles(C.T->lmax, C.l3max_eff, C.R, k, C.banded);
+    for (int k = C.nb - 1; k > b; --k) n += band_num_tiles(C.T->lmax, C.l3max_eff, C.R, k, C.banded, C.row_lo, C.row_hi);
     return (int)n;
 }
 
@@ -505,6 +522,7 @@ cudaError_t coupling_sweep(const Call &C, int b0, int b1, cudaStream_t st)
     P.tile_off = all ? 0 : tiles_above(C, b1 - 1);
     P.wstride = WSET * (long long)T.nl_alloc;
     P.even_mask = ~1;
+    P.row_lo = C.row_lo; P.row_hi = C.row_hi; P.rows = C.rows ? 1 : 0;
     P.ostride = C.N * C.ld;
     const int n = all ? C.ntiles : tiles_above(C, b0 - 1) - P.tile_off;
     return launch_sweep(P, C.mask, C.nw, C.mask == M_TT ? 2 : C.spin, n, st);
@@ -558,6 +576,31 @@ int run_coupling(const tj_tables *tables, int lcut, const double *d_Wtt, const d
     coupling_end(C, st);
     return rc;
 }
+// full rows [row_lo, row_hi) of every requested block, compact outputs (tj_coupling_rows)
+int run_rows(const tj_tables *tables, const double *d_Wtt, const double *d_Wtp, const double *d_Wpp, int nW, int row_lo,
+             int row_hi, double *d_TT, double *d_TE, double *d_EE, double *d_BB, double *d_EB, cudaStream_t st)
+{
+    Call C;
+    int rc = coupling_begin(C, tables, -1, d_Wtt, d_Wtp, d_Wpp, nW, d_TT, d_TE, d_EE, d_BB, d_EB, st, 1, 2, row_lo, row_hi);
+    if (rc != TJ_OK) return rc;
+    prof_record(2, st);
+    cudaError_t e = coupling_sweep(C, 0, C.nb, st);
+    prof_record(3, st);
+    if (e == cudaSuccess) {
+        double *M[4] = {nullptr, nullptr, nullptr, nullptr};
+        int n = 0, bb_src = -1;
+        if (C.TT) M[n++] = C.TT;
+        if (C.TE) M[n++] = C.TE;
+        if (C.ee) { if (C.bb_copy) bb_src = n; M[n++] = C.ee; }
+        if (C.EB) M[n++] = C.EB;
+        e = launch_scale_rows(M, n, C.bb_copy, bb_src, (long long)(row_hi - row_lo), C.T->lmax, st);
+    }
+    prof_record(4, st);
+    if (e != cudaSuccess) rc = cuda_fail(e, "tj_coupling_rows");
+    coupling_end(C, st);
+    return rc;
+}
+
 // paper-literal ablation (tj_literal.cu): prefold the windows, then one thread per pair
 int run_literal(const tj_tables *tables, const double *d_Wtt, const double *d_Wpp, int nW, double *d_TT, double *d_EE,
                 cudaStream_t st)

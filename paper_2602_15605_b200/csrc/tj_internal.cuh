@@ -43,8 +43,17 @@ constexpr int M_TT = 1, M_TE = 2, M_EE = 4, M_EB = 8;
 
 __host__ __device__ inline int num_bands(int lmax, int R) { return (lmax + R) / R; }  // ceil((lmax+1)/R)
 
-// columns c needed by row band `band`: c_lo = a; c_hi as below (inclusive)
-__host__ __device__ inline int band_c_hi(int lmax, int l3max, int R, int band, bool banded)
+// Columns c needed by row band `band` (rows a..a+R-1, a = band*R): c_lo .. c_hi inclusive.
+// A call may be restricted to the full rows [row_lo, row_hi) of the matrices (tj_coupling_rows; the whole matrix is
+// row_lo = 0, row_hi = lmax+1): a band that reaches into the block needs all its columns c >= a (upper part of those
+// rows); a band entirely above the block contributes only the mirrored entries, i.e. the pairs whose l2 = c-i lies in
+// the block; bands below the block contribute nothing.
+__host__ __device__ inline int band_c_lo(int R, int band, int row_lo)
+{
+    int a = band * R;
+    return (a + R - 1 >= row_lo) ? a : row_lo;
+}
+__host__ __device__ inline int band_c_hi(int lmax, int l3max, int R, int band, bool banded, int row_lo, int row_hi)
 {
     int a = band * R;
     int hi = lmax + R - 1;
@@ -52,13 +61,15 @@ __host__ __device__ inline int band_c_hi(int lmax, int l3max, int R, int band, b
         long long alt = (long long)a + 2 * R - 2 + l3max;
         if (alt < hi) hi = (int)alt;
     }
+    if (a + R - 1 < row_lo && row_hi + R - 2 < hi) hi = row_hi + R - 2;
     return hi;
 }
-__host__ __device__ inline int band_num_tiles(int lmax, int l3max, int R, int band, bool banded)
+__host__ __device__ inline int band_num_tiles(int lmax, int l3max, int R, int band, bool banded, int row_lo, int row_hi)
 {
-    int a = band * R;
-    int hi = band_c_hi(lmax, l3max, R, band, banded);
-    return hi >= a ? (hi - a + SWEEP_THREADS) / SWEEP_THREADS : 0;
+    if (band * R >= row_hi) return 0;
+    int lo = band_c_lo(R, band, row_lo);
+    int hi = band_c_hi(lmax, l3max, R, band, banded, row_lo, row_hi);
+    return hi >= lo ? (hi - lo + SWEEP_THREADS) / SWEEP_THREADS : 0;
 }
 
 struct Tables {
@@ -81,6 +92,8 @@ struct SweepParams {
     const int *tile_start;          // [nbands+1] exclusive prefix of tiles per band, bands in DESCENDING order
     int lmax, l3max, nbands, lcut;  // lcut < 0: dense storage
     int even_mask;                  // ~1 (see the sweep: keeps a parity out of the compiler's sight)
+    int row_lo, row_hi;             // full rows [row_lo, row_hi) are computed (whole matrix: 0, lmax+1)
+    int rows;                       // 1: compact row-block outputs [(l1-row_lo)*ld + l2], direct AND mirrored entries stored
     int tile_off;                   // first tile of this launch in the descending-band prefix (row-chunked launches)
     long long ld;                   // row stride of the outputs
     long long wstride;              // multi-window: doubles between the prefolded arrays of consecutive window sets
@@ -103,7 +116,9 @@ struct WriterParams {
 cudaError_t launch_build_tables(const Tables &T, cudaStream_t st);
 cudaError_t launch_prepare(const Tables &T, const double *d_Wtt, const double *d_Wtp, const double *d_Wpp, int nW,
                            double *wtt, double *wtp, double *wpp, double *wA, double *wB, int *tile_start, int R,
-                           int l3max_eff, bool banded, cudaStream_t st);
+                           int l3max_eff, bool banded, int row_lo, int row_hi, cudaStream_t st);
+// row-block outputs: M[r][c] *= (2c+1) for the nmat blocks in M (rows x (lmax+1) each), bb = copy of M[bb_src] or NULL
+cudaError_t launch_scale_rows(double *const M[4], int nmat, double *bb, int bb_src, long long rows, int lmax, cudaStream_t st);
 int sweep_R(int mask, bool banded, int nw, int lmax);   // pairs per thread (= rows per band) of the sweep that serves `mask` for nw window sets
 cudaError_t launch_sweep(const SweepParams &P, int mask, int nw, int spin, int total_tiles, cudaStream_t st);
 cudaError_t launch_writer(const WriterParams &P, cudaStream_t st);

@@ -22,7 +22,7 @@ __global__ void __launch_bounds__(PREP_THREADS)
 prepare_kernel(const double *__restrict__ Wtt, const double *__restrict__ Wtp, const double *__restrict__ Wpp, int nW,
                double *wtt, double *wtp, double *wpp, double2 *wA, double2 *wB, const double *__restrict__ u3,
                int nl_alloc,
-               int *tile_start, int lmax, int l3max_eff, int R, int banded)
+               int *tile_start, int lmax, int l3max_eff, int R, int banded, int row_lo, int row_hi)
 {
     const double inv4pi = 0.079577471545947667884441881686257181;  // 1/(4 pi)
     const int lo = -GUARD_LO, hi = nl_alloc - GUARD_LO;
@@ -44,7 +44,7 @@ prepare_kernel(const double *__restrict__ Wtt, const double *__restrict__ Wtp, c
     const int chunk = (nb + PREP_THREADS - 1) / PREP_THREADS;
     const int k0 = threadIdx.x * chunk, k1 = min(nb, k0 + chunk);
     int sum = 0;
-    for (int k = k0; k < k1; ++k) sum += band_num_tiles(lmax, l3max_eff, R, nb - 1 - k, banded != 0);
+    for (int k = k0; k < k1; ++k) sum += band_num_tiles(lmax, l3max_eff, R, nb - 1 - k, banded != 0, row_lo, row_hi);
     part[threadIdx.x] = sum;
     __syncthreads();
     if (threadIdx.x == 0) {
@@ -56,7 +56,7 @@ prepare_kernel(const double *__restrict__ Wtt, const double *__restrict__ Wtp, c
     int run = part[threadIdx.x];
     for (int k = k0; k < k1; ++k) {
         tile_start[k] = run;
-        run += band_num_tiles(lmax, l3max_eff, R, nb - 1 - k, banded != 0);
+        run += band_num_tiles(lmax, l3max_eff, R, nb - 1 - k, banded != 0, row_lo, row_hi);
     }
 }
 
@@ -64,13 +64,13 @@ prepare_kernel(const double *__restrict__ Wtt, const double *__restrict__ Wtp, c
 
 cudaError_t launch_prepare(const Tables &T, const double *d_Wtt, const double *d_Wtp, const double *d_Wpp, int nW,
                            double *wtt, double *wtp, double *wpp, double *wA, double *wB, int *tile_start, int R,
-                           int l3max_eff, bool banded, cudaStream_t st)
+                           int l3max_eff, bool banded, int row_lo, int row_hi, cudaStream_t st)
 {
     int nb = (T.nl_alloc + PREP_THREADS - 1) / PREP_THREADS;
     if (nb > 64) nb = 64;
     prepare_kernel<<<nb, PREP_THREADS, 0, st>>>(d_Wtt, d_Wtp, d_Wpp, nW, wtt, wtp, wpp, (double2 *)wA, (double2 *)wB,
                                                  T.u3, T.nl_alloc, tile_start,
-                                                 T.lmax, l3max_eff, R, banded ? 1 : 0);
+                                                 T.lmax, l3max_eff, R, banded ? 1 : 0, row_lo, row_hi);
     return cudaGetLastError();
 }
 

@@ -155,7 +155,7 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB * (128 / SWEEP_THREADS)) s
     const int cb = tile - __ldg(P.tile_start + lo);
     const int a = band * R;
     const int lane = (int)(threadIdx.x & 31), warp = SWEEP_THREADS == 32 ? 0 : (int)(threadIdx.x >> 5);   // 0: keeps the warp's addresses CTA-uniform
-    const int cw = a + cb * SWEEP_THREADS + warp * 32;   // first column of the warp
+    const int cw = band_c_lo(R, band, P.row_lo) + cb * SWEEP_THREADS + warp * 32;   // first column of the warp
     const int c = cw + lane;
     const int sw = a + cw;                               // smallest s of the warp
 
@@ -341,10 +341,15 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB * (128 / SWEEP_THREADS)) s
             if (l2 >= l1 && l2 <= P.lmax && (P.lcut < 0 || l2 - l1 <= P.lcut)) {
                 const double sd = P.isd[l1] * P.isd[l2];
                 const long long col = P.lcut < 0 ? (long long)l2 : (long long)(l2 - l1 + P.lcut);
-                if (P.EB) {
+                if (P.EB && !P.rows) {
 #pragma unroll
                     for (int w = 0; w < NW; ++w)
                         P.EB[w * P.ostride + (long long)l1 * P.ld + col] = acc[w][i] * (0.25 * sd * sd);
+                }
+                if (P.EB && P.rows) {   // row block: Xi(l1,l2) goes to [l1][l2] and, mirrored, to [l2][l1], where inside
+                    const double v = acc[0][i] * (0.25 * sd * sd);
+                    if (l1 >= P.row_lo && l1 < P.row_hi) P.EB[(long long)(l1 - P.row_lo) * P.ld + l2] = v;
+                    if (l2 >= P.row_lo && l2 < P.row_hi && l2 != l1) P.EB[(long long)(l2 - P.row_lo) * P.ld + l1] = v;
                 }
             }
         }
@@ -518,12 +523,20 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB * (128 / SWEEP_THREADS)) s
                 const long long col = P.lcut < 0 ? (long long)l2 : (long long)(l2 - l1 + P.lcut);
                 const long long idx = (long long)l1 * P.ld + col;
                 const double sd = kA2 ? P.isd[l1] * P.isd[l2] : 0.0;
+                if (!P.rows) {
 #pragma unroll
-                for (int w = 0; w < NW; ++w) {
-                    const long long iw = idx + w * P.ostride;
-                    if (kTT && P.TT) P.TT[iw] = att[w][i];
-                    if (kTE && P.TE) P.TE[iw] = ate[w][i] * (0.5 * sd);
-                    if (kEE && P.EE) P.EE[iw] = aee[w][i] * (0.25 * sd * sd);
+                    for (int w = 0; w < NW; ++w) {
+                        const long long iw = idx + w * P.ostride;
+                        if (kTT && P.TT) P.TT[iw] = att[w][i];
+                        if (kTE && P.TE) P.TE[iw] = ate[w][i] * (0.5 * sd);
+                        if (kEE && P.EE) P.EE[iw] = aee[w][i] * (0.25 * sd * sd);
+                    }
+                } else {   // row block (see the odd branch)
+                    const bool in1 = l1 >= P.row_lo && l1 < P.row_hi, in2 = l2 >= P.row_lo && l2 < P.row_hi && l2 != l1;
+                    const long long i1 = (long long)(l1 - P.row_lo) * P.ld + l2, i2 = (long long)(l2 - P.row_lo) * P.ld + l1;
+                    if (kTT && P.TT) { const double v = att[0][i]; if (in1) P.TT[i1] = v; if (in2) P.TT[i2] = v; }
+                    if (kTE && P.TE) { const double v = ate[0][i] * (0.5 * sd); if (in1) P.TE[i1] = v; if (in2) P.TE[i2] = v; }
+                    if (kEE && P.EE) { const double v = aee[0][i] * (0.25 * sd * sd); if (in1) P.EE[i1] = v; if (in2) P.EE[i2] = v; }
                 }
             }
         }

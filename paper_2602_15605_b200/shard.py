@@ -33,3 +33,25 @@ def max_over_ranks(value: float, dist=None, device=None) -> float:
 def whole_job_throughput(units_per_rank: float, steps: int, ms_max: float, world: int) -> float:
     """units all ranks processed / the slowest rank's time (weak scaling, same work per rank)."""
     return world * units_per_rank * steps / (ms_max * 1e-3)
+
+
+def row_blocks(lmax: int, world: int) -> list[tuple[int, int]]:
+    """Cut the rows 0..lmax of ONE matrix into `world` contiguous blocks of (nearly) equal sweep work for
+    tj_coupling_rows (each GPU owns a row block, no exchange).  Work of row r = the pairs the
+    block sweeps for it: its upper-triangle part, (r+1) steps for each of the N-r columns l2 >= r, plus the mirrored
+    part, l+1 steps for each l < r.  Returns [(row_lo, row_hi), ...] covering 0..lmax+1; blocks may be empty
+    (row_lo == row_hi) only when world > lmax+1."""
+    if lmax < 0 or world <= 0:
+        raise ValueError("bad (lmax, world) = (%r, %r)" % (lmax, world))
+    N = lmax + 1
+    cost = [(r + 1) * (N - r) + r * (r + 1) // 2 for r in range(N)]
+    total = sum(cost)
+    cuts, acc, r = [0], 0, 0
+    for k in range(1, world):
+        target = total * k // world
+        while r < N and acc + cost[r] <= target:
+            acc += cost[r]
+            r += 1
+        cuts.append(r)
+    cuts.append(N)
+    return [(cuts[k], cuts[k + 1]) for k in range(world)]

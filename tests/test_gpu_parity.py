@@ -628,3 +628,54 @@ def test_multi_window_tt_only_bitwise_and_oracle():
         ref = oracle.coupling_full(lmax, 2 * lmax, Wtt[w], None, None)["TT"]
         assert_parity(out["TT"][w].cpu().numpy(), ref, "multi TT set %d" % w)
     T.close()
+
+
+# ---------------------------------------------------------------- row blocks
+@pytest.mark.parametrize("lmax", [150, 1003])
+def test_row_blocks_equal_rows_of_full_matrix_bitwise(lmax):
+    """tj_coupling_rows: any block of full rows, bit-identical to the same rows of tj_coupling_pol (blocks that
+    start/end inside a row band of the sweep, the first and the last rows, one row, everything)."""
+    import torch
+    wl = windows.config(1, lmax=lmax)
+    T = binding.build_tables(lmax)
+    W = [_t(w) for w in (wl.Wtt, wl.Wtp, wl.Wpp)]
+    full = binding.coupling_pol(T, *W)
+    tt = binding.coupling_tt(T, W[0])
+    torch.cuda.synchronize()
+    N = lmax + 1
+    blocks = [(0, 1), (0, 7), (5, 6), (13, 37), (24, 48), (N - 1, N), (N // 2 - 3, N // 2 + 40), (N - 29, N), (0, N)]
+    for r0, r1 in blocks:
+        pre = {k: torch.full((r1 - r0, N), float("nan"), dtype=torch.float64, device="cuda") for k in BLOCKS}
+        got = binding.coupling_rows(T, *W, r0, r1, out=pre)
+        only = binding.coupling_rows(T, W[0], None, None, r0, r1, want=("TT",))
+        torch.cuda.synchronize()
+        for k in BLOCKS:
+            assert torch.equal(got[k], full[k][r0:r1]), (k, r0, r1)
+        assert torch.equal(only["TT"], tt[r0:r1]), (r0, r1)
+    with pytest.raises(binding.TJError):
+        binding.coupling_rows(T, *W, 5, 5)
+    with pytest.raises(binding.TJError):
+        binding.coupling_rows(T, *W, 0, N + 1)
+    T.close()
+
+
+def test_row_blocks_config1_against_oracle_and_cover():
+    """Config 1 cut into 4 work-balanced row blocks (shard.row_blocks): the blocks tile the matrix, each block
+    against the oracle on sampled rows."""
+    import torch
+    from paper_2602_15605_b200 import shard
+    wl = windows.config(1)
+    N = wl.lmax + 1
+    T = binding.build_tables(wl.lmax)
+    W = [_t(w) for w in (wl.Wtt, wl.Wtp, wl.Wpp)]
+    cuts = shard.row_blocks(wl.lmax, 4)
+    assert cuts[0][0] == 0 and cuts[-1][1] == N and all(a[1] == b[0] for a, b in zip(cuts, cuts[1:]))
+    for r0, r1 in cuts:
+        got = binding.coupling_rows(T, *W, r0, r1)
+        torch.cuda.synchronize()
+        rows = np.unique(np.array([r0, (r0 + r1) // 2, r1 - 1], dtype=np.int32))
+        ref = oracle.coupling_rows(wl.lmax, wl.l3max, wl.Wtt, wl.Wtp, wl.Wpp, rows)
+        for k in BLOCKS:
+            assert_parity(got[k][torch.as_tensor(rows - r0, dtype=torch.int64).cuda()].cpu().numpy(), ref[k],
+                          "rows [%d,%d) %s" % (r0, r1, k))
+    T.close()
