@@ -71,3 +71,19 @@ def test_assign_window_sets_edge_cases():
     with pytest.raises(ValueError):
         shard.assign_window_sets(3, 2, 2)
     assert shard.max_over_ranks(3.5, None) == 3.5
+
+
+def test_row_blocks_partition_is_a_balanced_cover():
+    from paper_2602_15605_b200 import shard
+    for lmax, world in [(0, 1), (2, 5), (100, 3), (2000, 4), (10000, 8)]:
+        N = lmax + 1
+        cuts = shard.row_blocks(lmax, world)
+        assert len(cuts) == world and cuts[0][0] == 0 and cuts[-1][1] == N
+        assert all(a[1] == b[0] and a[0] <= a[1] for a, b in zip(cuts, cuts[1:]))
+        cost = [(r + 1) * (N - r) + r * (r + 1) // 2 for r in range(N)]
+        loads = [sum(cost[a:b]) for a, b in cuts]
+        assert sum(loads) == sum(cost)
+        if N >= 50 * world:
+            assert max(loads) <= 1.02 * sum(cost) / world + max(cost)
+    with pytest.raises(ValueError):
+        shard.row_blocks(10, 0)
