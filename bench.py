@@ -168,6 +168,9 @@ def main():
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json configs index (headline: 3)")
     ap.add_argument("--nwin", type=int, default=1,
                     help="window sets per step through tj_coupling_multi (default 1: the headline tj_coupling_pol step)")
+    ap.add_argument("--split-rows", action="store_true",
+                    help="N > 1: cut ONE matrix set into N work-balanced row blocks, one per rank (tj_coupling_rows, no "
+                         "exchange; strong scaling) instead of one independent window set per rank (the default, weak)")
     ap.add_argument("--ablation", action="store_true",
                     help="also time tj_coupling_literal (the paper's per-pair Eq. 10 / Eq. 16 evaluation) on the same workload")
     ap.add_argument("--no-e2e", action="store_true")
@@ -198,7 +201,8 @@ def main():
     binding.load_library()   # fails loudly if the CUDA library is missing: no fallback
 
     base = windows.config(args.config)
-    if world > 1 and not base.band:
+    split = bool(args.split_rows) and not base.band and base.pol and args.nwin <= 1
+    if world > 1 and not base.band and not split:
         # each rank: its own window set of the same recipe (independent problems, weak scaling)
         spec = {1: ((0.7, 30.0, 2.5), (0.5, 50.0, 3.0), False), 2: ((0.6, 40.0, 2.2), (0.45, 60.0, 2.8), True),
                 3: ((0.4, 80.0, 2.0), (0.35, 100.0, 2.4), False)}.get(args.config)
@@ -226,10 +230,19 @@ def main():
         out = {k: torch.empty((nwin, N, width), dtype=torch.float64, device="cuda") for k in blocks}
     else:
         out = {k: torch.empty((N, width), dtype=torch.float64, device="cuda") for k in blocks}
+    row_lo, row_hi = 0, N
+    if split:
+        # one problem, rank r computes the full rows of block r; the e2e leg is not defined for it
+        row_lo, row_hi = shard.row_blocks(wl.lmax, world)[rank]
+        args.no_e2e = True
+        out = {k: torch.empty((max(row_hi - row_lo, 1), N), dtype=torch.float64, device="cuda") for k in blocks}
     flush = torch.empty(512 * 1024 * 1024 // 8, dtype=torch.float64, device="cuda")
 
     def step():
-        if nwin > 1:
+        if split:
+            if row_hi > row_lo:
+                binding.coupling_rows(T, *dW, row_lo, row_hi, want=blocks, out=out)
+        elif nwin > 1:
             binding.coupling_multi(T, *dW, want=blocks, out=out)
         elif wl.band:
             binding.coupling_band(T, wl.l3max, *dW, want=blocks, out=out)
@@ -268,13 +281,21 @@ def main():
     step_ms = [a.elapsed_time(b) for a, b in ev]
     total_ms = float(sum(step_ms))
     total_ms = shard.max_over_ranks(total_ms, dist, "cuda")
-    value = shard.whole_job_throughput(terms, args.steps, total_ms, world)
+    # split rows: the job is ONE matrix set (its terms counted once); else every rank does `terms`
+    value = shard.whole_job_throughput(terms, args.steps, total_ms, 1 if split else world)
 
     # ---- roofline of the dominant kernel (the sweep), timed live with the library's CUDA events ----
     sweep_ms = statistics.mean(k[1] for k in kern)
     prep_ms = statistics.mean(k[0] for k in kern)
     writer_ms = statistics.mean(k[2] for k in kern)
-    if wl.pol:
+    if split and world > 1:
+        # rank 0's launch sweeps its own upper-triangle rows plus the pairs (l1 < row_lo, l2 in the block)
+        nb = row_hi - row_lo
+        Eb = sum((l + 1) * (N - l) for l in range(row_lo, row_hi)) + nb * (row_lo * (row_lo + 1) // 2)
+        Ob = sum(l * (N - l) for l in range(row_lo, row_hi)) + nb * (row_lo * (row_lo - 1) // 2)
+        alg_instr = INSTR_EVEN_POL * Eb + INSTR_ODD * Ob
+        alg_flops = 12 * Eb + 6 * Ob
+    elif wl.pol:
         alg_instr = INSTR_EVEN_POL * E + INSTR_ODD * O
         alg_flops = 12 * E + 6 * O
     else:
@@ -364,12 +385,13 @@ def main():
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": total_ms / args.steps, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "scaling": "strong" if split else "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": wl.name, "lmax": wl.lmax, "l3max": wl.l3max, "blocks": "+".join(blocks), "window_sets_per_step": nwin,
                        "terms_even": E, "terms_odd": O, "pairs_upper": P,
-                       "pairs_per_s": world * P * args.steps / (total_ms * 1e-3),
+                       "pairs_per_s": (1 if split else world) * P * args.steps / (total_ms * 1e-3),
                        "l2": "512 MB flush written between timed steps; each step also writes %.1f GB of output" % (bytes_out / 1e9),
-                       "parallelism": "1 problem per GPU" if world > 1 else "single GPU"},
+                       "parallelism": ("one matrix set cut into %d row blocks (tj_coupling_rows), rank 0 rows [%d,%d)" % (world, row_lo, row_hi))
+                       if split else ("1 problem per GPU" if world > 1 else "single GPU")},
             "roofline": roofline, "cpu_baseline": cpu_baseline, "e2e": e2e, "ablation": ablation,
             # per window set one prepare + one writer launch, per group of sets (3, or 2 + 2 for a remainder of 4) one sweep
             "gpu_launches": (2 * nwin + ngroups) * args.steps if nwin > 1

@@ -128,7 +128,7 @@ __device__ __forceinline__ int slice_bytes(int i0, int n)
 // (DESIGN.md 3 item 6):  even step: (-1 1 0) = X d / (2 sqrt(u1 u2)), d = u3-u1-u2, so the
 // "TE" slot accumulates W' X^2 d and the "EE" slot W' X^2 d^2; odd step: (-1 1 0)^2 = Z^2 / (4 u1 u2), so the "EB"
 // slot accumulates W' Z^2; P.isd then holds 1/sqrt(u_l) and the epilogue scales are the same expressions.
-template <int R, int MASK, int TS, int MINB, bool PIPE, int NW, int SPIN>
+template <int R, int MASK, int TS, int MINB, bool PIPE, int NW, int SPIN, bool ROWS>
 __global__ void __launch_bounds__(SWEEP_THREADS, MINB * (128 / SWEEP_THREADS)) sweep_tma_kernel(const __grid_constant__ SweepParams P)
 {
     constexpr bool kTT = (MASK & M_TT) != 0, kTE = (MASK & M_TE) != 0, kEE = (MASK & M_EE) != 0,
@@ -155,7 +155,7 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB * (128 / SWEEP_THREADS)) s
     const int cb = tile - __ldg(P.tile_start + lo);
     const int a = band * R;
     const int lane = (int)(threadIdx.x & 31), warp = SWEEP_THREADS == 32 ? 0 : (int)(threadIdx.x >> 5);   // 0: keeps the warp's addresses CTA-uniform
-    const int cw = band_c_lo(R, band, P.row_lo) + cb * SWEEP_THREADS + warp * 32;   // first column of the warp
+    const int cw = (ROWS ? band_c_lo(R, band, P.row_lo) : a) + cb * SWEEP_THREADS + warp * 32;   // first column of the warp
     const int c = cw + lane;
     const int sw = a + cw;                               // smallest s of the warp
 
@@ -341,12 +341,12 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB * (128 / SWEEP_THREADS)) s
             if (l2 >= l1 && l2 <= P.lmax && (P.lcut < 0 || l2 - l1 <= P.lcut)) {
                 const double sd = P.isd[l1] * P.isd[l2];
                 const long long col = P.lcut < 0 ? (long long)l2 : (long long)(l2 - l1 + P.lcut);
-                if (P.EB && !P.rows) {
+                if (P.EB && !ROWS) {
 #pragma unroll
                     for (int w = 0; w < NW; ++w)
                         P.EB[w * P.ostride + (long long)l1 * P.ld + col] = acc[w][i] * (0.25 * sd * sd);
                 }
-                if (P.EB && P.rows) {   // row block: Xi(l1,l2) goes to [l1][l2] and, mirrored, to [l2][l1], where inside
+                if (P.EB && ROWS) {   // row block: Xi(l1,l2) goes to [l1][l2] and, mirrored, to [l2][l1], where inside
                     const double v = acc[0][i] * (0.25 * sd * sd);
                     if (l1 >= P.row_lo && l1 < P.row_hi) P.EB[(long long)(l1 - P.row_lo) * P.ld + l2] = v;
                     if (l2 >= P.row_lo && l2 < P.row_hi && l2 != l1) P.EB[(long long)(l2 - P.row_lo) * P.ld + l1] = v;
@@ -523,7 +523,7 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB * (128 / SWEEP_THREADS)) s
                 const long long col = P.lcut < 0 ? (long long)l2 : (long long)(l2 - l1 + P.lcut);
                 const long long idx = (long long)l1 * P.ld + col;
                 const double sd = kA2 ? P.isd[l1] * P.isd[l2] : 0.0;
-                if (!P.rows) {
+                if (!ROWS) {
 #pragma unroll
                     for (int w = 0; w < NW; ++w) {
                         const long long iw = idx + w * P.ostride;
@@ -543,18 +543,18 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB * (128 / SWEEP_THREADS)) s
     }
 }
 
-template <int R, int MASK, int TS, int MINB, bool PIPE, int NW = 1, int SPIN = 2>
+template <int R, int MASK, int TS, int MINB, bool PIPE, int NW = 1, int SPIN = 2, bool ROWS = false>
 cudaError_t launch_one(const SweepParams &P, int total_tiles, cudaStream_t st)
 {
     if (total_tiles <= 0) return cudaSuccess;
     constexpr int NWARP = SWEEP_THREADS / 32;
     constexpr size_t smem = (size_t)NWARP * NBUF * Lay<TS, NW, MASK != M_TT>::BUFD * 8 + (size_t)NWARP * NBUF * 8;
     if (smem > 48 * 1024) {   // opt-in beyond the default limit (per device, so not cached; one-warp CTAs stay below it)
-        cudaError_t e = cudaFuncSetAttribute(sweep_tma_kernel<R, MASK, TS, MINB, PIPE, NW, SPIN>,
+        cudaError_t e = cudaFuncSetAttribute(sweep_tma_kernel<R, MASK, TS, MINB, PIPE, NW, SPIN, ROWS>,
                                              cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
     }
-    sweep_tma_kernel<R, MASK, TS, MINB, PIPE, NW, SPIN><<<total_tiles, SWEEP_THREADS, smem, st>>>(P);
+    sweep_tma_kernel<R, MASK, TS, MINB, PIPE, NW, SPIN, ROWS><<<total_tiles, SWEEP_THREADS, smem, st>>>(P);
     return cudaGetLastError();
 }
 
@@ -579,6 +579,16 @@ cudaError_t launch_sweep(const SweepParams &P, int mask, int nw, int spin, int t
 {
     constexpr int POL = M_TE | M_EE | M_EB, ALL = M_TT | POL;
     const bool banded = P.lcut >= 0;
+    if (P.rows) {   // row blocks (tj_coupling_rows): dense, one window set, spin 2
+        if (banded || nw != 1 || spin != 2) return cudaErrorInvalidValue;
+        switch (mask) {
+            case M_TT: return P.lmax >= LMAX_LONG ? launch_one<R_TT_LONG, M_TT, 64, 2, false, 1, 2, true>(P, total_tiles, st)
+                                                  : launch_one<R_TT, M_TT, 48, 3, false, 1, 2, true>(P, total_tiles, st);
+            case POL: return launch_one<R_POL, POL, TS_DENSE_LONG, 2, TJ_PIPE, 1, 2, true>(P, total_tiles, st);
+            case ALL: return launch_one<R_POL, ALL, TS_DENSE_LONG, 2, TJ_PIPE, 1, 2, true>(P, total_tiles, st);
+            default: return cudaErrorInvalidValue;
+        }
+    }
     if (spin == 1) {   // dense, one window set; TT-only requests use the spin-independent TT sweep below
         if (banded || nw != 1) return cudaErrorInvalidValue;
         if (mask == ALL) return launch_one<R_POL, ALL, TS_DENSE_SHORT, 2, TJ_PIPE, 1, 1>(P, total_tiles, st);
