@@ -62,7 +62,7 @@ namespace {
 #endif
 constexpr int TS_DENSE_LONG = TJ_TS_LONG, TS_DENSE_SHORT = TJ_TS_SHORT;
 #ifndef TJ_TS_BAND
-#define TJ_TS_BAND 32
+#define TJ_TS_BAND 64
 #endif
 constexpr int NBUF = 2;   // buffers per warp
 constexpr int PAD = 2;    // doubles in front of each slice: the software-pipelined read of "step TS" lands here
