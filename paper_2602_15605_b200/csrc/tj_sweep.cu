@@ -139,6 +139,8 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB * (128 / SWEEP_THREADS)) s
     using L = Lay<TS, NW, kPk>;
     constexpr int NWL = 2 * (TS - 1) + 32;   // l3 values one stage of a warp covers
     static_assert(TS % R == 0 && TS % 2 == 0, "stage length: a multiple of R and even");
+    static_assert(2 * (R + TS) + 8 <= GUARD_LO, "a warp reads down to index -2(R+TS) of a window: the low guard band must cover it");
+    static_assert(R + 64 + 8 <= GUARD_HI, "columns up to lmax+R-1+31 and their sums a+c: the high guard band must cover them");
     static_assert(R % 2 == 0, "even R: every block of R steps starts at an even step, which aligns the paired loads of the step factor");
 
     extern __shared__ __align__(128) unsigned char smem_raw[];
