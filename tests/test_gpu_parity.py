@@ -679,3 +679,41 @@ def test_row_blocks_config1_against_oracle_and_cover():
             assert_parity(got[k][torch.as_tensor(rows - r0, dtype=torch.int64).cuda()].cpu().numpy(), ref[k],
                           "rows [%d,%d) %s" % (r0, r1, k))
     T.close()
+
+
+def test_adjudication_against_exact_racah_sums():
+    """Where the GPU path and the oracle disagree most the exact Racah symbols decide.  At lmax = 192 (config-1
+    recipe) the largest relative disagreement, 2e-12, is the TE entry (14,135), whose terms cancel to 1e-4 of their
+    size; the others are squeezed and diagonal entries.  Each sum is re-done from exact squared
+    symbols (big-integer rationals, rounded once per term, math.fsum) and both sides are measured against it on the
+    scale of the terms: the table path is the more accurate side."""
+    import torch
+    from racah import threej_sq_sign
+    wl = windows.config(1, lmax=192)
+    got = run_pol(wl.lmax, wl.l3max, wl.Wtt, wl.Wtp, wl.Wpp)
+    pairs = [(14, 135), (192, 192), (191, 192), (150, 190), (100, 101), (2, 192), (64, 64), (157, 154)]
+    l1s = np.array([p[0] for p in pairs], dtype=np.int32)
+    l2s = np.array([p[1] for p in pairs], dtype=np.int32)
+    ora = oracle.coupling_pairs(wl.l3max, wl.Wtt, wl.Wtp, wl.Wpp, l1s, l2s)
+    worst_gpu = worst_ora = 0.0
+    for n, (l1, l2) in enumerate(pairs):
+        terms = {"TT": [], "TE": [], "EE": [], "EB": []}
+        for l3 in range(abs(l1 - l2), l1 + l2 + 1):
+            w = 2 * l3 + 1
+            s0, g0 = threej_sq_sign(l1, l2, l3, 0, 0, 0)
+            s2, g2 = threej_sq_sign(l1, l2, l3, -2, 2, 0)
+            terms["TT"].append(w * wl.Wtt[l3] * float(s0))
+            if (l1 + l2 + l3) % 2 == 0:
+                terms["EE"].append(w * wl.Wpp[l3] * float(s2))
+                terms["TE"].append(w * wl.Wtp[l3] * g0 * g2 * math.sqrt(float(s0) * float(s2)))
+            else:
+                terms["EB"].append(w * wl.Wpp[l3] * float(s2))
+        pref = (2 * l2 + 1) / (4 * math.pi)
+        for k, t in terms.items():
+            ex = pref * math.fsum(t)
+            scale = pref * math.fsum(abs(x) for x in t)
+            worst_gpu = max(worst_gpu, abs(got[k][l1, l2] - ex) / scale)
+            worst_ora = max(worst_ora, abs(ora[k][n] - ex) / scale)
+    print("vs exact Racah sums, on the scale of the terms: GPU worst %.2e, oracle worst %.2e" % (worst_gpu, worst_ora))
+    assert worst_gpu < 2e-15
+    assert worst_ora < 1e-13
