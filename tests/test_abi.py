@@ -85,3 +85,27 @@ def test_binding_fails_loudly_without_library(monkeypatch, tmp_path):
     monkeypatch.setattr(binding, "_SO", str(tmp_path / "nope.so"))
     with pytest.raises(binding.TJError):
         binding.load_library()
+
+
+def test_header_is_plain_c_and_links(tmp_path):
+    """include/tj.h compiles as C (no torch or C++ types at the boundary) and a C program links against libtj.so
+    and calls the host-side entry points."""
+    import subprocess
+    src = tmp_path / "use_tj.c"
+    src.write_text(
+        '#include "tj.h"\n#include <stdio.h>\n'
+        "int main(void) {\n"
+        "  int lo, hi, n;\n"
+        "  if (tj_l3_range(3, 5, 100, 0, &lo, &hi, &n) != TJ_OK) return 1;\n"
+        "  if (lo != 2 || hi != 8 || n != 4) return 2;\n"
+        "  if (tj_l3_range(3, 5, 100, 1, &lo, &hi, &n) != TJ_OK || lo != 3 || hi != 7 || n != 3) return 3;\n"
+        "  if (tj_build_tables(-1, 0, 0, 0) != TJ_EINVAL) return 4;\n"
+        '  printf("%s\\n", tj_strerror(TJ_OK));\n'
+        "  return 0;\n}\n")
+    exe = tmp_path / "use_tj"
+    libdir = os.path.dirname(binding.library_path())
+    inc = os.path.join(os.path.dirname(libdir), "include")
+    subprocess.run(["gcc", "-std=c99", "-Wall", "-Werror", "-I", inc, str(src), "-o", str(exe), "-L", libdir, "-l:libtj.so",
+                    "-Wl,-rpath," + libdir], check=True)
+    p = subprocess.run([str(exe)], capture_output=True, text=True)
+    assert p.returncode == 0 and p.stdout.strip() == "ok", (p.returncode, p.stdout, p.stderr)
