@@ -24,7 +24,7 @@ constexpr int GUARD_HI = 768;
 // blockIdx alone, so ptxas keeps it in the uniform datapath instead of broadcasting five registers per bulk copy
 // (measured at config 3: 137.3 ms with 128 threads, 136.3 with 64, 133.5 with 32).
 constexpr int SWEEP_THREADS = 32;
-// (TJ_R_POL, TJ_TS_LONG/TJ_TS_SHORT/TJ_PIPE and TJ_TS_BAND are tuning hooks: `TJ_NVCC_EXTRA="-DTJ_R_POL=14 ..." python -m
+// (TJ_R_POL, TJ_TS_LONG/TJ_TS_SHORT/TJ_PIPE/TJ_MINB_POL and TJ_TS_BAND are tuning hooks: `TJ_NVCC_EXTRA="-DTJ_R_POL=14 ..." python -m
 // paper_2602_15605_b200.build --force` rebuilds with another geometry; the defaults are the measured optimum)
 #ifndef TJ_R_POL
 #define TJ_R_POL 12

@@ -60,6 +60,9 @@ namespace {
 #define TJ_TS_SHORT 48
 #define TJ_PIPE true
 #endif
+#ifndef TJ_MINB_POL
+#define TJ_MINB_POL 2
+#endif
 constexpr int TS_DENSE_LONG = TJ_TS_LONG, TS_DENSE_SHORT = TJ_TS_SHORT;
 #ifndef TJ_TS_BAND
 #define TJ_TS_BAND 64
@@ -608,12 +611,12 @@ cudaError_t launch_sweep(const SweepParams &P, int mask, int nw, int spin, int t
                                                  : launch_one<R_TT, M_TT, 48, 3, false>(P, total_tiles, st));
         case POL:
             return banded ? launch_one<R_POL_BAND, POL, TJ_TS_BAND, 3, false>(P, total_tiles, st)
-                          : (P.lmax >= LMAX_LONG ? launch_one<R_POL, POL, TS_DENSE_LONG, 2, TJ_PIPE>(P, total_tiles, st)
-                                                        : launch_one<R_POL, POL, TS_DENSE_SHORT, 2, TJ_PIPE>(P, total_tiles, st));
+                          : (P.lmax >= LMAX_LONG ? launch_one<R_POL, POL, TS_DENSE_LONG, TJ_MINB_POL, TJ_PIPE>(P, total_tiles, st)
+                                                        : launch_one<R_POL, POL, TS_DENSE_SHORT, TJ_MINB_POL, TJ_PIPE>(P, total_tiles, st));
         case ALL:
             return banded ? launch_one<R_POL_BAND, ALL, TJ_TS_BAND, 3, false>(P, total_tiles, st)
-                          : (P.lmax >= LMAX_LONG ? launch_one<R_POL, ALL, TS_DENSE_LONG, 2, TJ_PIPE>(P, total_tiles, st)
-                                                        : launch_one<R_POL, ALL, TS_DENSE_SHORT, 2, TJ_PIPE>(P, total_tiles, st));
+                          : (P.lmax >= LMAX_LONG ? launch_one<R_POL, ALL, TS_DENSE_LONG, TJ_MINB_POL, TJ_PIPE>(P, total_tiles, st)
+                                                        : launch_one<R_POL, ALL, TS_DENSE_SHORT, TJ_MINB_POL, TJ_PIPE>(P, total_tiles, st));
         default: return cudaErrorInvalidValue;
     }
 }
