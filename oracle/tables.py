@@ -6,6 +6,12 @@ PAPER.md:186: the method stores g(p), 1/g(p) and 1/(J+1) (J = 2p on the even-J b
 The values are exact rationals; `float(Fraction)` / Python's int true division round them
 correctly (round-half-even) to float64, so every entry returned here is the correctly rounded
 value of its definition.  Nothing here is shared with the CUDA table kernel.
+
+Pins (tests/test_oracle_tables.py, `-m "not gpu"`): numerator/denominator == (math.comb(2p,p), 4^p) as
+integers (every p <= 1500, strided to p = 32001); g(0..2) = 1, 1/2, 3/8 and Eq. 12 in exact Fractions;
+the convolution identity sum_k g(k) g(n-k) = 1; ln g against lgamma for EVERY p <= 32001; Stirling's limit
+g(p) sqrt(pi p) = 1 - 1/(8p) + ...; all five derived entries against exact Fractions (p <= 300) and against
+mpmath's gamma function at 60 digits (strided to p = 32001).  No function here is "parity unpinned".
 """
 from __future__ import annotations
 
