@@ -717,3 +717,165 @@ def test_adjudication_against_exact_racah_sums():
     print("vs exact Racah sums, on the scale of the terms: GPU worst %.2e, oracle worst %.2e" % (worst_gpu, worst_ora))
     assert worst_gpu < 2e-15
     assert worst_ora < 1e-13
+
+
+# ---------------------------------------------------------------- every shipped sweep variant has its own parity test
+@pytest.mark.parametrize("want", [("TT",), ("TE", "EE", "EB"), ("TE", "EE", "BB", "EB")])
+@pytest.mark.parametrize("lmax,lcut", [(500, 40), (333, 101)])
+def test_band_partial_requests_against_oracle(lmax, lcut, want):
+    """tj_coupling_band with TT alone and with the polarised blocks alone (their own sweep variants), element-wise
+    against the oracle, and bitwise against the same blocks of the all-blocks band call."""
+    import torch
+    rng = np.random.default_rng(lmax + lcut)
+    W = [np.abs(rng.standard_normal(lcut + 1)) * np.exp(-np.arange(lcut + 1) / 30.0) for _ in range(3)]
+    T = binding.build_tables(lmax)
+    N, width = lmax + 1, 2 * lcut + 1
+    pre = {k: torch.full((N, width), float("nan"), dtype=torch.float64, device="cuda") for k in want}
+    got = binding.coupling_band(T, lcut, _t(W[0]) if "TT" in want else None, _t(W[1]) if "TE" in want else None,
+                                _t(W[2]) if set(want) & {"EE", "BB", "EB"} else None, want=want, out=pre)
+    allb = binding.coupling_band(T, lcut, *[_t(w) for w in W])
+    torch.cuda.synchronize()
+    ref = oracle.coupling_band(lmax, lcut, *W)
+    for k in want:
+        assert_parity(got[k].cpu().numpy(), ref[k], "band %r %s" % (want, k))
+        assert torch.equal(got[k], allb[k]), (want, k)
+    T.close()
+
+
+def test_band_partial_requests_full_size_cfg4_sampled():
+    """Config 4 (lmax 15000, L_cut 300) with TT alone and with the polarised blocks alone: sampled against the oracle."""
+    import torch
+    wl = windows.config(4)
+    lcut = wl.l3max
+    T = binding.build_tables(wl.lmax)
+    l1, l2 = _sample_pairs(wl.lmax, 1200, 105, band=lcut)
+    ref = oracle.coupling_pairs(lcut, wl.Wtt, wl.Wtp, wl.Wpp, l1, l2)
+    i1 = torch.as_tensor(l1.astype(np.int64)).cuda()
+    io = torch.as_tensor((l2.astype(np.int64) - l1 + lcut)).cuda()
+    for want in (("TT",), ("TE", "EE", "EB")):
+        got = binding.coupling_band(T, lcut, _t(wl.Wtt) if "TT" in want else None, _t(wl.Wtp) if "TE" in want else None,
+                                    _t(wl.Wpp) if "EE" in want else None, want=want)
+        torch.cuda.synchronize()
+        for k in want:
+            assert bool(torch.isfinite(got[k]).all())
+            assert_parity(got[k][i1, io].cpu().numpy(), ref[k], "cfg4 %r %s" % (want, k))
+    T.close()
+
+
+def test_row_blocks_pol_only_against_oracle():
+    """tj_coupling_rows without TT (its own sweep variant): sampled rows of config 1 against the oracle, bitwise
+    against the rows of the full polarised call."""
+    import torch
+    wl = windows.config(1)
+    N = wl.lmax + 1
+    T = binding.build_tables(wl.lmax)
+    W = [_t(w) for w in (wl.Wtt, wl.Wtp, wl.Wpp)]
+    want = ("TE", "EE", "BB", "EB")
+    full = binding.coupling_pol(T, None, W[1], W[2], want=want)
+    for r0, r1 in ((0, 90), (700, 1291), (N - 45, N)):
+        pre = {k: torch.full((r1 - r0, N), float("nan"), dtype=torch.float64, device="cuda") for k in want}
+        got = binding.coupling_rows(T, None, W[1], W[2], r0, r1, want=want, out=pre)
+        torch.cuda.synchronize()
+        rows = np.unique(np.array([r0, (r0 + r1) // 2, r1 - 1], dtype=np.int32))
+        ref = oracle.coupling_rows(wl.lmax, wl.l3max, None, wl.Wtp, wl.Wpp, rows)
+        for k in want:
+            assert torch.equal(got[k], full[k][r0:r1]), (k, r0, r1)
+            assert_parity(got[k][torch.as_tensor(rows - r0, dtype=torch.int64).cuda()].cpu().numpy(), ref[k],
+                          "pol-only rows [%d,%d) %s" % (r0, r1, k))
+    T.close()
+
+
+def test_row_blocks_tt_only_long_geometry():
+    """tj_coupling_rows with TT alone at lmax >= 4096 (the long TT-only geometry): sampled pairs against the oracle,
+    whole blocks bitwise against tj_coupling_tt."""
+    import torch
+    wl = windows.config(2, lmax=4300)
+    N = wl.lmax + 1
+    T = binding.build_tables(wl.lmax)
+    Wtt = _t(wl.Wtt)
+    tt = binding.coupling_tt(T, Wtt)
+    rng = np.random.default_rng(77)
+    for r0, r1 in ((0, 257), (2011, 3100), (N - 300, N)):
+        got = binding.coupling_rows(T, Wtt, None, None, r0, r1, want=("TT",))["TT"]
+        torch.cuda.synchronize()
+        assert torch.equal(got, tt[r0:r1]), (r0, r1)
+        l1 = rng.integers(r0, r1, 400).astype(np.int32)
+        l2 = rng.integers(0, N, 400).astype(np.int32)
+        ref = oracle.coupling_pairs(wl.l3max, wl.Wtt, None, None, l1, l2)
+        g = got[torch.as_tensor(l1.astype(np.int64) - r0).cuda(), torch.as_tensor(l2.astype(np.int64)).cuda()].cpu().numpy()
+        assert_parity(g, ref["TT"], "TT-only rows [%d,%d)" % (r0, r1))
+    T.close()
+
+
+# ---------------------------------------------------------------- T4 bookkeeping THROUGH THE KERNEL: every l3 slot of every pair
+def _oracle_ranges(lmax, l3max):
+    """(lo, hi, n) of the l3 sum of every pair, per parity of l1+l2+l3: the ORACLE's integer bookkeeping."""
+    out = []
+    for par in (0, 1):
+        r = np.array([[oracle.l3_range(l1, l2, l3max, par) for l2 in range(lmax + 1)] for l1 in range(lmax + 1)])
+        out.append((r[..., 0], r[..., 1], r[..., 2]))
+    return out
+
+
+def _expected_support(ranges, L):
+    """Which (l1,l2) have l3 = L among their terms, for even and for odd l1+l2+L."""
+    return tuple((n > 0) & (lo <= L) & (L <= hi) & ((L - lo) % 2 == 0) for lo, hi, n in ranges)
+
+
+@pytest.mark.parametrize("lmax,l3max", [(48, 96), (48, 61), (33, 20)])
+def test_spike_every_l3_slot_dense(lmax, l3max):
+    """W = delta_{l,L} for EVERY L = 0..l3max: an entry is non-zero iff l3 = L is one of the terms the kernel adds for
+    that pair, so the zero pattern of these launches is the kernel's own l3 bookkeeping, slot by slot, compared with
+    the oracle's integer ranges (PAPER.md:133-151; :251 for the truncated l3max)."""
+    import torch
+    T = binding.build_tables(lmax, l3max)
+    l1, l2 = np.indices((lmax + 1, lmax + 1))
+    pol = (l1 >= 2) & (l2 >= 2)
+    ranges = _oracle_ranges(lmax, l3max)
+    for L in range(l3max + 1):
+        W = _t(windows.spike(l3max, L))
+        K = {k: v.cpu().numpy() for k, v in binding.coupling_pol(T, W, W, W).items()}
+        ev, od = _expected_support(ranges, L)
+        assert np.all(K["TT"][~ev] == 0.0) and np.all(K["TT"][ev] > 0.0), L
+        for k in ("TE", "EE", "BB"):
+            assert np.all(K[k][~(ev & pol)] == 0.0), (k, L)
+        assert np.all(K["EB"][~(od & pol)] == 0.0), L
+        assert np.all(K["EE"][ev & pol] >= 0.0) and np.all(K["EB"][od & pol] >= 0.0)
+        # the spin-2 symbol has accidental zeros (A = 0), so "non-zero inside" is checked through the oracle's values
+        ref = oracle.coupling_full(lmax, l3max, *(3 * [windows.spike(l3max, L)]))
+        for k in BLOCKS:
+            assert_parity(K[k], ref[k], "spike L=%d %s" % (L, k))
+            assert np.all((K[k] != 0.0) | (np.abs(ref[k]) < 1e-13)), (k, L)
+    T.close()
+
+
+@pytest.mark.parametrize("lmax,lcut", [(48, 30), (40, 7)])
+def test_spike_every_l3_slot_banded(lmax, lcut):
+    """The same through tj_coupling_band: every L = 0..lcut."""
+    import torch
+    T = binding.build_tables(lmax)
+    N, width = lmax + 1, 2 * lcut + 1
+    l1 = np.repeat(np.arange(N), width).reshape(N, width)
+    l2 = l1 + np.arange(-lcut, lcut + 1)[None, :]
+    ok = (l2 >= 0) & (l2 <= lmax)
+    pol = (l1 >= 2) & (l2 >= 2)
+    ranges = _oracle_ranges(lmax, lcut)
+    for L in range(lcut + 1):
+        Wn = np.zeros(lcut + 1)
+        Wn[L] = 1.0
+        W = _t(Wn)
+        pre = {k: torch.full((N, width), float("nan"), dtype=torch.float64, device="cuda") for k in BLOCKS}
+        K = {k: v.cpu().numpy() for k, v in binding.coupling_band(T, lcut, W, W, W, out=pre).items()}
+        ev, od = _expected_support(ranges, L)
+        evb = np.zeros((N, width), dtype=bool)
+        odb = np.zeros((N, width), dtype=bool)
+        evb[ok] = ev[l1[ok], l2[ok]]
+        odb[ok] = od[l1[ok], l2[ok]]
+        assert np.all(K["TT"][~evb] == 0.0) and np.all(K["TT"][evb] > 0.0), L
+        for k in ("TE", "EE", "BB"):
+            assert np.all(K[k][~(evb & pol)] == 0.0), (k, L)
+        assert np.all(K["EB"][~(odb & pol)] == 0.0), L
+        ref = oracle.coupling_band(lmax, lcut, Wn, Wn, Wn)
+        for k in BLOCKS:
+            assert_parity(K[k], ref[k], "band spike L=%d %s" % (L, k))
+    T.close()
