@@ -81,6 +81,11 @@ struct Call {
     unsigned char *scratch = nullptr;
     double *wtt = nullptr, *wtp = nullptr, *wpp = nullptr, *wA = nullptr, *wB = nullptr;
     int *tile_start = nullptr;
+    // band-limited calls (diagonal tiling): the sweep leaves Xi in a transposed scratch xit[k][delta*ldT + l1]
+    // (k-th requested block in the order TT, TE, EE, EB), the band writer scales / mirrors it into the outputs
+    double *xit[4] = {nullptr, nullptr, nullptr, nullptr};
+    long long ldT = 0;
+    int dmax = 0;
 };
 
 // One coupling call on device pointers.  lcut < 0: dense (l3max = handle's); else banded with l3 <= lcut.
@@ -449,7 +454,14 @@ int coupling_begin(Call &C, const tj_tables *tables, int lcut, const double *d_W
     C.row_lo = C.rows ? row_lo : 0;
     C.row_hi = C.rows ? row_hi : T.lmax + 1;
     C.ld = C.banded ? (long long)(2 * lcut + 1) : C.N;
-    C.ntiles = total_tiles(T.lmax, C.l3max_eff, C.R, C.banded, C.row_lo, C.row_hi);
+    C.dmax = C.banded ? (lcut < T.lmax ? lcut : T.lmax) : 0;
+    C.ldT = (C.N + 15) & ~15LL;
+    if (C.banded) {
+        const long long n = (long long)diag_num_groups(C.dmax, C.R) * diag_num_blocks(T.lmax, C.R);
+        C.ntiles = n > 0x7fffffffLL ? -1 : (int)n;
+    } else {
+        C.ntiles = total_tiles(T.lmax, C.l3max_eff, C.R, false, C.row_lo, C.row_hi);
+    }
     if (C.ntiles < 0) return TJ_EINVAL;
     C.nb = num_bands(T.lmax, C.R);
     C.ntile_w = (int)((C.N + 31) / 32);
@@ -458,8 +470,12 @@ int coupling_begin(Call &C, const tj_tables *tables, int lcut, const double *d_W
     // per window set: three plain prefolded arrays + two arrays of pairs (7 nl_alloc doubles)
     const size_t wbytes = sizeof(double) * WSET * (size_t)T.nl_alloc * (size_t)nw;
     const size_t tbytes = sizeof(int) * (size_t)(C.nb + 1 + 1);
-    const size_t tb_al = (tbytes + 15) & ~(size_t)15;
-    TJ_CUDA(cudaMallocAsync((void **)&C.scratch, wbytes + tb_al, st), "coupling/scratch");
+    const size_t tb_al = (tbytes + 127) & ~(size_t)127;
+    int nxit = 0;
+    if (C.banded) nxit = (C.TT ? 1 : 0) + (C.TE ? 1 : 0) + (C.ee ? 1 : 0) + (C.EB ? 1 : 0);
+    const size_t xper = (size_t)(C.dmax + 1) * (size_t)C.ldT;   // doubles per transposed Xi block
+    TJ_CUDA(cudaMallocAsync((void **)&C.scratch, wbytes + tb_al + sizeof(double) * xper * (size_t)nxit, st), "coupling/scratch");
+    for (int k = 0; k < nxit; ++k) C.xit[k] = (double *)(C.scratch + wbytes + tb_al) + xper * (size_t)k;
     C.wtt = (double *)C.scratch + GUARD_LO;
     C.wtp = C.wtt + T.nl_alloc;
     C.wpp = C.wtp + T.nl_alloc;
@@ -476,23 +492,6 @@ int coupling_begin(Call &C, const tj_tables *tables, int lcut, const double *d_W
                            C.banded, C.row_lo, C.row_hi, st);
     }
     prof_record(1, st);
-    if (e == cudaSuccess && C.banded) {
-        // slots of the band whose l2 falls outside 0..lmax are 0: they lie in the first and the last lcut rows, which
-        // are cleared here; every other slot is a valid pair and is written by the sweep (l2 >= l1) or the writer (mirror)
-        const size_t per = (size_t)C.N * (size_t)C.ld;
-        const size_t head = (size_t)(lcut < C.N ? lcut : C.N);           // rows [0, head)
-        const size_t tail0 = (size_t)(C.N - lcut > (long long)head ? C.N - lcut : (long long)head);   // rows [tail0, N)
-        double *outs[5] = {d_TT, d_TE, d_EE, d_BB, d_EB};
-        for (int k = 0; k < 5 && e == cudaSuccess; ++k) {
-            if (!outs[k]) continue;
-            for (int w = 0; w < nw && e == cudaSuccess; ++w) {
-                double *m = outs[k] + (size_t)w * per;
-                if (head) e = cudaMemsetAsync(m, 0, sizeof(double) * head * (size_t)C.ld, st);
-                if (e == cudaSuccess && (size_t)C.N > tail0)
-                    e = cudaMemsetAsync(m + tail0 * (size_t)C.ld, 0, sizeof(double) * ((size_t)C.N - tail0) * (size_t)C.ld, st);
-            }
-        }
-    }
     if (e != cudaSuccess) { cudaFreeAsync(C.scratch, st); C.scratch = nullptr; return cuda_fail(e, "coupling/prepare"); }
     return TJ_OK;
 }
@@ -518,6 +517,15 @@ cudaError_t coupling_sweep(const Call &C, int b0, int b1, cudaStream_t st)
     P.TT = C.TT; P.TE = C.TE; P.EE = C.ee; P.EB = C.EB;
     P.tile_start = C.tile_start;
     P.lmax = T.lmax; P.l3max = C.l3max_eff; P.nbands = C.nb; P.lcut = C.banded ? C.lcut : -1; P.ld = C.ld;
+    P.nd = diag_num_blocks(T.lmax, C.R);
+    if (C.banded) {   // diagonal tiling: Xi goes to the transposed scratch
+        int k = 0;
+        if (C.TT) P.TT = C.xit[k++];
+        if (C.TE) P.TE = C.xit[k++];
+        if (C.ee) P.EE = C.xit[k++];
+        if (C.EB) P.EB = C.xit[k++];
+        P.ld = C.ldT;
+    }
     const bool all = (b0 == 0 && b1 == C.nb);
     P.tile_off = all ? 0 : tiles_above(C, b1 - 1);
     P.wstride = WSET * (long long)T.nl_alloc;
@@ -531,6 +539,19 @@ cudaError_t coupling_sweep(const Call &C, int b0, int b1, cudaStream_t st)
 // scale + mirror of the 32-row tile rows [I0, I1)
 cudaError_t coupling_write(const Call &C, int I0, int I1, cudaStream_t st)
 {
+    if (C.banded) {
+        BandWriterParams B;
+        memset(&B, 0, sizeof(B));
+        int n = 0;
+        B.bb_src = -1;
+        if (C.TT) { B.X[n] = C.xit[n]; B.M[n] = C.TT; ++n; }
+        if (C.TE) { B.X[n] = C.xit[n]; B.M[n] = C.TE; ++n; }
+        if (C.ee) { if (C.bb_copy) { B.bb = C.bb_copy; B.bb_src = n; } B.X[n] = C.xit[n]; B.M[n] = C.ee; ++n; }
+        if (C.EB) { B.X[n] = C.xit[n]; B.M[n] = C.EB; ++n; }
+        B.nmat = n;
+        B.lmax = C.T->lmax; B.lcut = C.lcut; B.dmax = C.dmax; B.ldT = C.ldT; B.ld = C.ld;
+        return launch_band_writer(B, st);
+    }
     WriterParams W;
     memset(&W, 0, sizeof(W));
     int n = 0;
@@ -540,10 +561,9 @@ cudaError_t coupling_write(const Call &C, int I0, int I1, cudaStream_t st)
     if (C.ee) { if (C.bb_copy) { W.bb = C.bb_copy; W.bb_src = n; } W.M[n++] = C.ee; }
     if (C.EB) W.M[n++] = C.EB;
     W.nmat = n;
-    W.lmax = C.T->lmax; W.lcut = C.banded ? C.lcut : -1; W.ld = C.ld;
+    W.lmax = C.T->lmax; W.lcut = -1; W.ld = C.ld;
     W.ntile = C.ntile_w;
-    const int tb = (C.lcut + 31) / 32 + 1;
-    W.tile_band = (C.banded && tb < W.ntile - 1) ? tb : W.ntile - 1;
+    W.tile_band = W.ntile - 1;
     W.I0 = I0; W.I1 = I1;
     cudaError_t e = cudaSuccess;
     for (int w = 0; w < C.nw && e == cudaSuccess; ++w) {

@@ -31,7 +31,8 @@ constexpr int SWEEP_THREADS = 32;
 #endif
 constexpr int R_POL = TJ_R_POL;           // pairs per thread, fused TT+TE+EE(+EB) sweep, dense storage
 constexpr int R_POL_BAND = 8;       // same, band-limited (short sweeps)
-constexpr int R_TT = 16;            // pairs per thread, TT-only sweep (short or band-limited sweeps)
+constexpr int R_TT = 16;            // pairs per thread, TT-only sweep (short sweeps)
+constexpr int R_TT_BAND = 16;       // same, band-limited
 constexpr int R_TT_LONG = 32;       // same, dense sweeps at lmax >= LMAX_LONG (measured at lmax = 10^4: 24.9 -> 22.8 ms)
 constexpr int LMAX_LONG = 4096;     // from here on a dense sweep uses the long-sweep geometry (R_TT_LONG; 96-step stages)
 constexpr int R_MULTI2 = 8;         // pairs per thread, 2 window sets per sweep (tj_coupling_multi)
@@ -72,6 +73,25 @@ __host__ __device__ inline int band_num_tiles(int lmax, int l3max, int R, int ba
     return hi >= lo ? (hi - lo + SWEEP_THREADS) / SWEEP_THREADS : 0;
 }
 
+// ---- diagonal tiling of a band |l1-l2| <= dmax (band-limited calls) -----------------------------
+// A warp tile is (delta group, diagonal block n): lane j of the warp owns the R pairs (a+j+i, a+j+d0-i), i = 0..R-1,
+// a = 32 n - (R-1): all on ONE anti-diagonal per lane, delta = l2-l1 = d0-2i the same in every lane.  With l3 <= lcut
+// a pair has floor((lcut-delta)/2)+1 even steps whatever its l1, so all 32 lanes of a warp (and all R pairs of a
+// thread, up to R-1-i steps) have the same step count: no lane waits for another (the column-major tiling of the
+// dense sweep loses ~16 of <= lcut/2 steps to the spread of s inside a warp).  Groups hold R deltas of one parity:
+// group 2m+p covers delta = p + 2Rm + 2i', i' = 0..R-1; groups are issued in ascending delta = descending work.
+__host__ __device__ inline int diag_d0(int R, int grp) { return (grp & 1) + 2 * R * (grp >> 1) + 2 * (R - 1); }
+__host__ __device__ inline int diag_num_groups(int dmax, int R)
+{
+    const int n0 = dmax / 2 + 1, n1 = (dmax + 1) / 2;   // even / odd deltas in 0..dmax
+    return (n0 + R - 1) / R + (n1 + R - 1) / R;
+}
+__host__ __device__ inline int diag_num_blocks(int lmax, int R) { return (lmax + R + 31) / 32; }
+
+// the sweep instantiation a launch used (for the roofline label of bench.py, tj_profile_geometry)
+struct SweepGeometry { int R, mask, TS, minb, pipe, nw, spin, rows, diag, tiles; };
+extern thread_local SweepGeometry g_last_sweep;
+
 struct Tables {
     int lmax, l3max, pmax;          // p-tables hold p = 0..pmax = 2*lmax+1
     int np_alloc;                   // doubles per p-table incl. guards
@@ -95,6 +115,7 @@ struct SweepParams {
     int row_lo, row_hi;             // full rows [row_lo, row_hi) are computed (whole matrix: 0, lmax+1)
     int rows;                       // 1: compact row-block outputs [(l1-row_lo)*ld + l2], direct AND mirrored entries stored
     int tile_off;                   // first tile of this launch in the descending-band prefix (row-chunked launches)
+    int nd;                         // diagonal tiling: diagonal blocks per delta group (grid = groups * nd)
     long long ld;                   // row stride of the outputs
     long long wstride;              // multi-window: doubles between the prefolded arrays of consecutive window sets
     long long ostride;              // multi-window: doubles between the output matrices of consecutive window sets
@@ -112,6 +133,17 @@ struct WriterParams {
     int I0, I1;                     // tile rows [I0, I1) of this launch (row-chunked launches; whole matrix: 0, ntile)
 };
 
+// band-limited calls: transposed Xi scratch -> banded storage (tj_writer.cu)
+struct BandWriterParams {
+    const double *X[4];             // Xi blocks, X[delta*ldT + l1] = Xi(l1, l1+delta), delta = 0..dmax
+    double *M[4];                   // banded outputs, M[l1*ld + (l2-l1+lcut)]
+    int nmat;
+    double *bb;                     // if non-NULL: receives a copy of M[bb_src]
+    int bb_src;
+    int lmax, lcut, dmax;           // dmax = min(lcut, lmax)
+    long long ldT, ld;              // ld = 2*lcut+1
+};
+
 // kernels / launchers (defined in the .cu files)
 cudaError_t launch_build_tables(const Tables &T, cudaStream_t st);
 cudaError_t launch_prepare(const Tables &T, const double *d_Wtt, const double *d_Wtp, const double *d_Wpp, int nW,
@@ -122,6 +154,7 @@ cudaError_t launch_scale_rows(double *const M[4], int nmat, double *bb, int bb_s
 int sweep_R(int mask, bool banded, int nw, int lmax);   // pairs per thread (= rows per band) of the sweep that serves `mask` for nw window sets
 cudaError_t launch_sweep(const SweepParams &P, int mask, int nw, int spin, int total_tiles, cudaStream_t st);
 cudaError_t launch_writer(const WriterParams &P, cudaStream_t st);
+cudaError_t launch_band_writer(const BandWriterParams &P, cudaStream_t st);
 cudaError_t launch_literal(const Tables &T, const double *wtt, const double *wpp, double *TT, double *EE, int l3max,
                            cudaStream_t st);   // paper-literal ablation kernel (tj_literal.cu)
 cudaError_t launch_fp64_probe(int iters, double *d_sink, int blocks, int threads, cudaStream_t st);

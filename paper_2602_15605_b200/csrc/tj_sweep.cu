@@ -105,7 +105,7 @@ template <int TS, int NW, bool PK> struct Lay {
     static constexpr int CA = PAD + TS + 2;            // row ring / step factor
     static constexpr int CB = PAD + TS + 32 + 2;       // column ring / h
     static constexpr int CW = PAD + 2 * TS + 32 + 2;   // windows, u3
-    static constexpr int OA = 0, OG = OA + CA, OB = OG + CA, OH = OB + CB;
+    static constexpr int OA = 0, OG = OA + CA, OB = OG + CB, OH = OB + CB;   // OG: CB doubles (the diagonal tiling reads g[t] per lane)
     static constexpr int OW0 = OH + CB;                // TT-only sweep: the plain W'_TT slices, one per window set
     // polarised sweeps read the windows as pairs (prepare_kernel): (W'_TT, W'_TP)[l] and (W'_PP, u_l)[l], one array
     // of 2*CW doubles per window set each, in the same region (the TT-only sweep keeps the plain W'_TT slot OW0)
@@ -131,7 +131,7 @@ __device__ __forceinline__ int slice_bytes(int i0, int n)
 // (DESIGN.md 3 item 6):  even step: (-1 1 0) = X d / (2 sqrt(u1 u2)), d = u3-u1-u2, so the
 // "TE" slot accumulates W' X^2 d and the "EE" slot W' X^2 d^2; odd step: (-1 1 0)^2 = Z^2 / (4 u1 u2), so the "EB"
 // slot accumulates W' Z^2; P.isd then holds 1/sqrt(u_l) and the epilogue scales are the same expressions.
-template <int R, int MASK, int TS, int MINB, bool PIPE, int NW, int SPIN, bool ROWS>
+template <int R, int MASK, int TS, int MINB, bool PIPE, int NW, int SPIN, bool ROWS, bool DIAG>
 __global__ void __launch_bounds__(SWEEP_THREADS, MINB * (128 / SWEEP_THREADS)) sweep_tma_kernel(const __grid_constant__ SweepParams P)
 {
     constexpr bool kTT = (MASK & M_TT) != 0, kTE = (MASK & M_TE) != 0, kEE = (MASK & M_EE) != 0,
@@ -141,6 +141,9 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB * (128 / SWEEP_THREADS)) s
     constexpr bool kPk = MASK != M_TT;   // windows and u3 come as pairs (wA, wB)
     using L = Lay<TS, NW, kPk>;
     constexpr int NWL = 2 * (TS - 1) + 32;   // l3 values one stage of a warp covers
+    // diagonal tiling: the step factor g[t+j] is the per-lane slice and the column ring g[c-i-t] a broadcast
+    constexpr int NG = DIAG ? TS + 31 : TS, NB = DIAG ? TS : TS + 31;
+    constexpr int LG = DIAG ? 1 : 0, LB = DIAG ? 0 : 1;   // which of the two a lane offsets by its index
     static_assert(TS % R == 0 && TS % 2 == 0, "stage length: a multiple of R and even");
     static_assert(2 * (R + TS) + 8 <= GUARD_LO, "a warp reads down to index -2(R+TS) of a window: the low guard band must cover it");
     static_assert(R + 64 + 8 <= GUARD_HI, "columns up to lmax+R-1+31 and their sums a+c: the high guard band must cover them");
@@ -149,20 +152,33 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB * (128 / SWEEP_THREADS)) s
     extern __shared__ __align__(128) unsigned char smem_raw[];
     constexpr int NWARP = SWEEP_THREADS / 32;
 
-    // ---- tile decode: binary search of blockIdx.x in the descending-band prefix ----
-    const int tile = (int)blockIdx.x + P.tile_off;
-    int lo = 0, hi = P.nbands;
-    while (hi - lo > 1) {
-        int mid = (lo + hi) >> 1;
-        if (__ldg(P.tile_start + mid) <= tile) lo = mid; else hi = mid;
-    }
-    const int band = P.nbands - 1 - lo;
-    const int cb = tile - __ldg(P.tile_start + lo);
-    const int a = band * R;
+    static_assert(!DIAG || (SWEEP_THREADS == 32 && NW == 1 && SPIN == 2 && !ROWS), "diagonal tiling: one warp, one window set");
     const int lane = (int)(threadIdx.x & 31), warp = SWEEP_THREADS == 32 ? 0 : (int)(threadIdx.x >> 5);   // 0: keeps the warp's addresses CTA-uniform
-    const int cw = (ROWS ? band_c_lo(R, band, P.row_lo) : a) + cb * SWEEP_THREADS + warp * 32;   // first column of the warp
+    int a, cw;   // lane 0's first row and column
+    if (DIAG) {
+        // ---- diagonal tiling (band-limited calls, tj_internal.cuh): tile = (delta group, diagonal block) ----
+        const int grp = (int)blockIdx.x / P.nd, n = (int)blockIdx.x - grp * P.nd;
+        a = 32 * n - (R - 1);
+        cw = a + diag_d0(R, grp);
+    } else {
+        // ---- tile decode: binary search of blockIdx.x in the descending-band prefix ----
+        const int tile = (int)blockIdx.x + P.tile_off;
+        int lo = 0, hi = P.nbands;
+        while (hi - lo > 1) {
+            int mid = (lo + hi) >> 1;
+            if (__ldg(P.tile_start + mid) <= tile) lo = mid; else hi = mid;
+        }
+        const int band = P.nbands - 1 - lo;
+        const int cb = tile - __ldg(P.tile_start + lo);
+        a = band * R;
+        cw = (ROWS ? band_c_lo(R, band, P.row_lo) : a) + cb * SWEEP_THREADS + warp * 32;   // first column of the warp
+    }
+    // the thread's pairs are (al+i, c-i).  Dense tiling: lanes run along the column, every lane has the rows a..a+R-1.
+    // Diagonal tiling: lane j is lane 0 shifted by (j, j), and walks the steps t+j while lane 0 walks t, so that every
+    // lane has the same number of steps; all table offsets below are lane 0's, the per-lane shift is in the slices.
     const int c = cw + lane;
-    const int sw = a + cw;                               // smallest s of the warp
+    const int al = DIAG ? a + lane : a;
+    const int sw = a + cw;                               // smallest s of the warp (diagonal tiling: lane 0's s)
 
     // a warp whose columns all lie beyond lmax has nothing to store
     if (cw - (R - 1) > P.lmax) return;
@@ -183,9 +199,11 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB * (128 / SWEEP_THREADS)) s
     // first steps rounded down to even (an extra step adds exact zeros): the step factor g[t] is then read two steps
     // per 16-byte load.  The mask is a kernel argument (always ~1) so that the compiler can NOT prove the parity and
     // pair the row-ring loads too: those go into fixed ring registers and a paired load costs two register moves.
-    tbo = tbo > 0 ? ((tbo + 1) >> 1) & P.even_mask : 0;
+    // Diagonal tiling: lane j starts j steps after lane 0, so lane 0 may start below 0 (the guard band of g[t] adds
+    // exact zeros there) but not below -32: then every lane starts at or below its own first step max(0, .).
+    tbo = DIAG ? max((tbo + 1) >> 1, -32) & P.even_mask : tbo > 0 ? ((tbo + 1) >> 1) & P.even_mask : 0;
     int tbe = sw - P.l3max;        // even: l3 = s-2t   <= l3max
-    tbe = tbe > 0 ? ((tbe + 1) >> 1) & P.even_mask : 0;
+    tbe = DIAG ? max((tbe + 1) >> 1, -32) & P.even_mask : tbe > 0 ? ((tbe + 1) >> 1) & P.even_mask : 0;
     const int nso = (kEB && tbo <= t_end) ? (t_end - tbo + TS) / TS : 0;
     const int nse = (kEven && tbe <= t_end) ? (t_end - tbe + TS) / TS : 0;
     const int ntot = nso + nse;
@@ -197,12 +215,12 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB * (128 / SWEEP_THREADS)) s
         const uint32_t bar = bar_s + 8u * b;
         if (q < nso) {
             const int t0 = tbo + q * TS, tl = t0 + TS - 1;
-            uint32_t bytes = slice_bytes(a - tl, TS) + slice_bytes(t0, TS) + slice_bytes(cw - R + 1 - tl, TS + 31) +
+            uint32_t bytes = slice_bytes(a - tl, TS) + slice_bytes(t0, NG) + slice_bytes(cw - R + 1 - tl, NB) +
                              slice_bytes(sw - tl, TS + 31) + NW * (2 * NWL * 8);
             mbar_expect_tx(bar, bytes);
             slice(buf, L::OA, P.gA, a - tl, TS, bar);
-            slice(buf, L::OG, P.gB, t0, TS, bar);
-            slice(buf, L::OB, P.gA, cw - R + 1 - tl, TS + 31, bar);
+            slice(buf, L::OG, P.gB, t0, NG, bar);
+            slice(buf, L::OB, P.gA, cw - R + 1 - tl, NB, bar);
             slice(buf, L::OH, P.ginv, sw - tl, TS + 31, bar);
 #pragma unroll
             for (int w = 0; w < NW; ++w)   // pairs (W'_PP, u_l), l = l3lo .. l3lo+NWL-1: always 16-byte aligned
@@ -210,13 +228,13 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB * (128 / SWEEP_THREADS)) s
                          P.wB + w * P.wstride + 2 * (long long)(sw - 2 * tl - 1), 2 * NWL * 8, bar);
         } else {
             const int t0 = tbe + (q - nso) * TS, tl = t0 + TS - 1;
-            uint32_t bytes = slice_bytes(a - tl, TS) + slice_bytes(t0, TS) + slice_bytes(cw - R + 1 - tl, TS + 31) +
+            uint32_t bytes = slice_bytes(a - tl, TS) + slice_bytes(t0, NG) + slice_bytes(cw - R + 1 - tl, NB) +
                              slice_bytes(sw - tl, TS + 31) +
                              (kPk ? NW * 2 * (2 * NWL * 8) : NW * slice_bytes(sw - 2 * tl, NWL));
             mbar_expect_tx(bar, bytes);
             slice(buf, L::OA, P.g, a - tl, TS, bar);
-            slice(buf, L::OG, P.g, t0, TS, bar);
-            slice(buf, L::OB, P.g, cw - R + 1 - tl, TS + 31, bar);
+            slice(buf, L::OG, P.g, t0, NG, bar);
+            slice(buf, L::OB, P.g, cw - R + 1 - tl, NB, bar);
             slice(buf, L::OH, P.h, sw - tl, TS + 31, bar);
             if (kPk) {
 #pragma unroll
@@ -243,7 +261,7 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB * (128 / SWEEP_THREADS)) s
     if (kA2 || kEB) {
 #pragma unroll
         for (int i = 0; i < R; ++i) {
-            const double l1 = (double)(a + i), l2 = (double)(c - i);
+            const double l1 = (double)(al + i), l2 = (double)(c - i);
             const double u1 = l1 * (l1 + 1.0), u2 = l2 * (l2 + 1.0);
             c12[i] = SPIN == 2 ? u1 + u2 - 2.0 : u1 + u2 - 1.0;   // odd branch: e = u3 - c12 (spin 1: unused)
             kk[i] = __fma_rn(2.0 * u1, u2, 1.0);     // even branch: A2 = d1^2 - kk (spin 1: unused)
@@ -263,7 +281,7 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB * (128 / SWEEP_THREADS)) s
             double wa[R], wb[R];
             {   // ring start-up straight from global memory (once per warp)
                 const double *pa = P.gA + (a - tbo);
-                const double *pb = P.gA + (c - R + 1 - tbo);
+                const double *pb = P.gA + (c - LG * lane - R + 1 - tbo);
 #pragma unroll
                 for (int k = 1; k < R; ++k) wa[k] = __ldg(pa + k);
 #pragma unroll
@@ -272,8 +290,8 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB * (128 / SWEEP_THREADS)) s
             // consumer offsets: parity of each slice's first index is the same in every stage (TS even)
             const int tl0 = tbo + TS - 1;
             const int oa = L::OA + PAD + ((a - tl0) & 1) + (TS - 1);
-            const int og = L::OG + PAD + (tbo & 1);
-            const int ob = L::OB + PAD + ((cw - R + 1 - tl0) & 1) + (TS - 1) + lane;
+            const int og = L::OG + PAD + (tbo & 1) + LG * lane;
+            const int ob = L::OB + PAD + ((cw - R + 1 - tl0) & 1) + (TS - 1) + LB * lane;
             const int oh = L::OH + PAD + ((sw - tl0) & 1) + (TS - 1) + lane;
             for (int k = 0; k < nso; ++k, ++q) {
                 // blocks of R steps this stage really has (the last stage is cut at the band's last step)
@@ -283,9 +301,9 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB * (128 / SWEEP_THREADS)) s
                 const double *sb = wbuf + b * L::BUFD;
                 const double *pa = sb + oa, *pg = sb + og, *pb = sb + ob, *ph = sb + oh;
                 // pairs (W'_PP, u_l) at l3 = s-2t-1: lane's element of step t0+j is 2(TS-1)+lane-2j
-                const double2 *pB = reinterpret_cast<const double2 *>(sb + L::OPB + 2 * PAD) + 2 * (TS - 1) + lane;
+                const double2 *pB = reinterpret_cast<const double2 *>(sb + L::OPB + 2 * PAD) + 2 * (TS - 1) + LB * lane;
                 double xa = pa[0], xb = pb[0], xh = ph[0];
-                double2 xg2 = *reinterpret_cast<const double2 *>(pg);   // g[t] of steps 0, 1
+                double2 xg2 = DIAG ? make_double2(pg[0], 0.0) : *reinterpret_cast<const double2 *>(pg);   // g[t] of steps 0, 1
                 double xg = xg2.x;
                 double xw[NW], xu;
                 {
@@ -309,7 +327,8 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB * (128 / SWEEP_THREADS)) s
                         // the warp-uniform step factor comes two steps per 16-byte load (the first step is even).  The
                         // same for the row ring costs more than it saves: its values go into fixed ring registers,
                         // so half of each pair needs a register move (two instructions) to get there.
-                        if (u % 2 == 0) xg = xg2.y;
+                        if (DIAG) xg = pg[u + 1];   // per lane: plain loads
+                        else if (u % 2 == 0) xg = xg2.y;
                         else { xg2 = *reinterpret_cast<const double2 *>(pg + (u + 1)); xg = xg2.x; }
                         {
                             const double2 v0 = pB[-2 * (u + 1)];
@@ -342,14 +361,16 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB * (128 / SWEEP_THREADS)) s
         // epilogue: Xi_EB = S_EB / (4 D)
 #pragma unroll
         for (int i = 0; i < R; ++i) {
-            const int l1 = a + i, l2 = c - i;
-            if (l2 >= l1 && l2 <= P.lmax && (P.lcut < 0 || l2 - l1 <= P.lcut)) {
+            const int l1 = al + i, l2 = c - i;
+            if (l2 >= l1 && l2 <= P.lmax && (P.lcut < 0 || l2 - l1 <= P.lcut) && (!DIAG || l1 >= 0)) {
                 const double sd = P.isd[l1] * P.isd[l2];
-                const long long col = P.lcut < 0 ? (long long)l2 : (long long)(l2 - l1 + P.lcut);
+                // diagonal tiling: Xi goes to the transposed scratch [l2-l1][l1] (lanes = consecutive l1: coalesced)
+                const long long idx = DIAG ? (long long)(l2 - l1) * P.ld + l1
+                                           : (long long)l1 * P.ld + (P.lcut < 0 ? (long long)l2 : (long long)(l2 - l1 + P.lcut));
                 if (P.EB && !ROWS) {
 #pragma unroll
                     for (int w = 0; w < NW; ++w)
-                        P.EB[w * P.ostride + (long long)l1 * P.ld + col] = acc[w][i] * (0.25 * sd * sd);
+                        P.EB[w * P.ostride + idx] = acc[w][i] * (0.25 * sd * sd);
                 }
                 if (P.EB && ROWS) {   // row block: Xi(l1,l2) goes to [l1][l2] and, mirrored, to [l2][l1], where inside
                     const double v = acc[0][i] * (0.25 * sd * sd);
@@ -379,7 +400,7 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB * (128 / SWEEP_THREADS)) s
             double wa[R], wb[R];
             {
                 const double *pa = P.g + (a - tbe);
-                const double *pb = P.g + (c - R + 1 - tbe);
+                const double *pb = P.g + (c - LG * lane - R + 1 - tbe);
 #pragma unroll
                 for (int k = 1; k < R; ++k) wa[k] = __ldg(pa + k);
 #pragma unroll
@@ -393,10 +414,10 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB * (128 / SWEEP_THREADS)) s
             for (int i = 0; i < R; ++i) { if (kTE) rA[i] = 0.0; if (kEE) rAA[i] = 0.0; }
             const int tl0 = tbe + TS - 1;
             const int oa = L::OA + PAD + ((a - tl0) & 1) + (TS - 1);
-            const int og = L::OG + PAD + (tbe & 1);
-            const int ob = L::OB + PAD + ((cw - R + 1 - tl0) & 1) + (TS - 1) + lane;
+            const int og = L::OG + PAD + (tbe & 1) + LG * lane;
+            const int ob = L::OB + PAD + ((cw - R + 1 - tl0) & 1) + (TS - 1) + LB * lane;
             const int oh = L::OH + PAD + ((sw - tl0) & 1) + (TS - 1) + lane;
-            const int ow = PAD + ((sw - 2 * tl0) & 1) + 2 * (TS - 1) + lane;
+            const int ow = PAD + ((sw - 2 * tl0) & 1) + 2 * (TS - 1) + LB * lane;
             for (int k = 0; k < nse; ++k, ++q) {
                 const int nblk = min(TS / R, (t_end - (tbe + k * TS) + R) / R);
                 const int b = q % NBUF;
@@ -405,10 +426,10 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB * (128 / SWEEP_THREADS)) s
                 const double *pa = sb + oa, *pg = sb + og, *pb = sb + ob, *ph = sb + oh;
                 const double *pwtt = sb + L::OW0 + ow;   // TT-only sweep: plain W'_TT
                 // polarised sweeps: pairs (W'_TT, W'_TP) and (W'_PP, u_l) at l3 = s-2t
-                const double2 *pA = reinterpret_cast<const double2 *>(sb + L::OPA + 2 * PAD) + 2 * (TS - 1) + lane;
-                const double2 *pB = reinterpret_cast<const double2 *>(sb + L::OPB + 2 * PAD) + 2 * (TS - 1) + lane;
+                const double2 *pA = reinterpret_cast<const double2 *>(sb + L::OPA + 2 * PAD) + 2 * (TS - 1) + LB * lane;
+                const double2 *pB = reinterpret_cast<const double2 *>(sb + L::OPB + 2 * PAD) + 2 * (TS - 1) + LB * lane;
                 double xa = pa[0], xb = pb[0], xh = ph[0];
-                double2 xg2 = *reinterpret_cast<const double2 *>(pg);   // g[t] of steps 0, 1
+                double2 xg2 = DIAG ? make_double2(pg[0], 0.0) : *reinterpret_cast<const double2 *>(pg);   // g[t] of steps 0, 1
                 double xg = xg2.x;
                 double xtt[NW], xtp[NW], xpp[NW], xu = 0.0;
                 // windows (and u3) of the step whose pair element sits `off` pairs from the lane's stage origin
@@ -447,7 +468,8 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB * (128 / SWEEP_THREADS)) s
                         // the warp-uniform step factor comes two steps per 16-byte load (the first step is even).  The
                         // same for the row ring costs more than it saves: its values go into fixed ring registers,
                         // so half of each pair needs a register move (two instructions) to get there.
-                        if (u % 2 == 0) xg = xg2.y;
+                        if (DIAG) xg = pg[u + 1];   // per lane: plain loads
+                        else if (u % 2 == 0) xg = xg2.y;
                         else { xg2 = *reinterpret_cast<const double2 *>(pg + (u + 1)); xg = xg2.x; }
                         load_w(-2 * (u + 1));
                         if (PIPE) {
@@ -523,10 +545,10 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB * (128 / SWEEP_THREADS)) s
         // epilogue: Xi_TT = S_TT; Xi_TE = S_TE/(2 sqrt D); Xi_EE = S_EE/(4 D)
 #pragma unroll
         for (int i = 0; i < R; ++i) {
-            const int l1 = a + i, l2 = c - i;
-            if (l2 >= l1 && l2 <= P.lmax && (P.lcut < 0 || l2 - l1 <= P.lcut)) {
-                const long long col = P.lcut < 0 ? (long long)l2 : (long long)(l2 - l1 + P.lcut);
-                const long long idx = (long long)l1 * P.ld + col;
+            const int l1 = al + i, l2 = c - i;
+            if (l2 >= l1 && l2 <= P.lmax && (P.lcut < 0 || l2 - l1 <= P.lcut) && (!DIAG || l1 >= 0)) {
+                const long long idx = DIAG ? (long long)(l2 - l1) * P.ld + l1
+                                           : (long long)l1 * P.ld + (P.lcut < 0 ? (long long)l2 : (long long)(l2 - l1 + P.lcut));
                 const double sd = kA2 ? P.isd[l1] * P.isd[l2] : 0.0;
                 if (!ROWS) {
 #pragma unroll
@@ -548,22 +570,25 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB * (128 / SWEEP_THREADS)) s
     }
 }
 
-template <int R, int MASK, int TS, int MINB, bool PIPE, int NW = 1, int SPIN = 2, bool ROWS = false>
+template <int R, int MASK, int TS, int MINB, bool PIPE, int NW = 1, int SPIN = 2, bool ROWS = false, bool DIAG = false>
 cudaError_t launch_one(const SweepParams &P, int total_tiles, cudaStream_t st)
 {
+    g_last_sweep = SweepGeometry{R, MASK, TS, MINB, PIPE ? 1 : 0, NW, SPIN, ROWS ? 1 : 0, DIAG ? 1 : 0, total_tiles};
     if (total_tiles <= 0) return cudaSuccess;
     constexpr int NWARP = SWEEP_THREADS / 32;
     constexpr size_t smem = (size_t)NWARP * NBUF * Lay<TS, NW, MASK != M_TT>::BUFD * 8 + (size_t)NWARP * NBUF * 8;
     if (smem > 48 * 1024) {   // opt-in beyond the default limit (per device, so not cached; one-warp CTAs stay below it)
-        cudaError_t e = cudaFuncSetAttribute(sweep_tma_kernel<R, MASK, TS, MINB, PIPE, NW, SPIN, ROWS>,
+        cudaError_t e = cudaFuncSetAttribute(sweep_tma_kernel<R, MASK, TS, MINB, PIPE, NW, SPIN, ROWS, DIAG>,
                                              cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
     }
-    sweep_tma_kernel<R, MASK, TS, MINB, PIPE, NW, SPIN, ROWS><<<total_tiles, SWEEP_THREADS, smem, st>>>(P);
+    sweep_tma_kernel<R, MASK, TS, MINB, PIPE, NW, SPIN, ROWS, DIAG><<<total_tiles, SWEEP_THREADS, smem, st>>>(P);
     return cudaGetLastError();
 }
 
 }  // namespace
+
+thread_local SweepGeometry g_last_sweep = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
 
 // Geometry per request: dense sweeps are long (up to lmax steps per pair), so the per-step
 // overhead (prefactors, table reads) is spread over R = 12 pairs at 2 CTAs/SM with stages of 96 (48) steps;
@@ -576,7 +601,7 @@ int sweep_R(int mask, bool banded, int nw, int lmax)
     if (mask == M_TT && nw > 1) return R_TT_MULTI;
     if (nw == 2) return R_MULTI2;
     if (nw == 3) return R_MULTI3;
-    if (mask == M_TT) return (!banded && lmax >= LMAX_LONG) ? R_TT_LONG : R_TT;
+    if (mask == M_TT) return banded ? R_TT_BAND : lmax >= LMAX_LONG ? R_TT_LONG : R_TT;
     return banded ? R_POL_BAND : R_POL;
 }
 
@@ -606,15 +631,15 @@ cudaError_t launch_sweep(const SweepParams &P, int mask, int nw, int spin, int t
     if (nw != 1) return cudaErrorInvalidValue;
     switch (mask) {
         case M_TT:
-            return banded ? launch_one<R_TT, M_TT, 32, 3, false>(P, total_tiles, st)
+            return banded ? launch_one<R_TT_BAND, M_TT, 32, 3, false, 1, 2, false, true>(P, total_tiles, st)
                           : (P.lmax >= LMAX_LONG ? launch_one<R_TT_LONG, M_TT, 64, 2, false>(P, total_tiles, st)
                                                  : launch_one<R_TT, M_TT, 48, 3, false>(P, total_tiles, st));
         case POL:
-            return banded ? launch_one<R_POL_BAND, POL, TJ_TS_BAND, 3, false>(P, total_tiles, st)
+            return banded ? launch_one<R_POL_BAND, POL, TJ_TS_BAND, 3, false, 1, 2, false, true>(P, total_tiles, st)
                           : (P.lmax >= LMAX_LONG ? launch_one<R_POL, POL, TS_DENSE_LONG, TJ_MINB_POL, TJ_PIPE>(P, total_tiles, st)
                                                         : launch_one<R_POL, POL, TS_DENSE_SHORT, TJ_MINB_POL, TJ_PIPE>(P, total_tiles, st));
         case ALL:
-            return banded ? launch_one<R_POL_BAND, ALL, TJ_TS_BAND, 3, false>(P, total_tiles, st)
+            return banded ? launch_one<R_POL_BAND, ALL, TJ_TS_BAND, 3, false, 1, 2, false, true>(P, total_tiles, st)
                           : (P.lmax >= LMAX_LONG ? launch_one<R_POL, ALL, TS_DENSE_LONG, TJ_MINB_POL, TJ_PIPE>(P, total_tiles, st)
                                                         : launch_one<R_POL, ALL, TS_DENSE_SHORT, TJ_MINB_POL, TJ_PIPE>(P, total_tiles, st));
         default: return cudaErrorInvalidValue;

@@ -9,8 +9,10 @@
 // (2 l2+1) M[l2][l1] agree to the last rounding.  BB, when requested next to EE, is written from the
 // same registers.
 //
-// Banded storage (step a7): address(l1,l2) = l1*ld + (l2-l1+lcut), valid for |l1-l2| <= lcut; only tile
-// pairs within the band are launched; slots whose l2 is outside 0..lmax were zeroed by the API.
+// Banded storage (step a7): address(l1,l2) = l1*ld + (l2-l1+lcut), valid for |l1-l2| <= lcut.  The band-limited
+// sweep (diagonal tiling) leaves Xi in a transposed scratch X[delta][l1]; band_writer_kernel turns 32x32 tiles of it
+// into full row segments of the band, direct (column lcut+delta) and mirrored (column lcut-delta), and writes 0.0
+// into the slots whose l2 falls outside 0..lmax -- every slot of the outputs is written exactly once.
 #include "tj_internal.cuh"
 
 namespace tj {
@@ -117,6 +119,57 @@ cudaError_t launch_scale_rows(double *const M[4], int nmat, double *bb, int bb_s
     long long nb = (total + 255) / 256;
     if (nb > 148 * 32) nb = 148 * 32;
     scale_rows_kernel<<<(unsigned)nb, 256, 0, st>>>(M[0], M[1], M[2], M[3], nmat, bb, bb_src, total, lmax + 1);
+    return cudaGetLastError();
+}
+
+// One CTA: rows r0..r0+31 of ONE banded output, deltas d0..d0+31.
+//   direct:  M[r][lcut+delta] = (2(r+delta)+1) Xi(r, r+delta)          source X[delta][r]
+//   mirror:  M[r][lcut-delta] = (2(r-delta)+1) Xi(r-delta, r)          source X[delta][r-delta]   (delta >= 1)
+// Both sources are read as 32 consecutive doubles per delta and transposed through shared memory.
+__global__ void __launch_bounds__(WT * WROWS) band_writer_kernel(const __grid_constant__ BandWriterParams P)
+{
+    __shared__ double td[WT][WT + 1], tm[WT][WT + 1];
+    const int tx = threadIdx.x, ty = threadIdx.y;
+    const int d0 = blockIdx.x * WT, r0 = blockIdx.y * WT, m = blockIdx.z;
+    const double *X = P.X[m];
+    double *M = P.M[m];
+    double *bb = (P.bb != nullptr && m == P.bb_src) ? P.bb : nullptr;
+#pragma unroll
+    for (int k = ty; k < WT; k += WROWS) {
+        const int delta = d0 + k;
+        const int l1d = r0 + tx, l1m = r0 - delta + tx;
+        const bool okd = delta <= P.dmax && l1d + delta <= P.lmax;
+        const bool okm = delta <= P.dmax && delta >= 1 && l1m >= 0 && l1m + delta <= P.lmax;
+        td[k][tx] = okd ? X[(long long)delta * P.ldT + l1d] : 0.0;
+        tm[k][tx] = okm ? X[(long long)delta * P.ldT + l1m] : 0.0;
+    }
+    __syncthreads();
+    const int delta = d0 + tx;
+    if (delta > P.lcut) return;
+#pragma unroll
+    for (int k = ty; k < WT; k += WROWS) {
+        const int r = r0 + k;
+        if (r > P.lmax) break;
+        const long long row = (long long)r * P.ld + P.lcut;
+        {   // out-of-range slots read 0.0 from the tile: 0.0 * (2 l2+1) = 0.0
+            const double v = td[tx][k] * (double)(2 * (r + delta) + 1);
+            M[row + delta] = v;
+            if (bb) bb[row + delta] = v;
+        }
+        if (delta >= 1) {
+            const double v = tm[tx][k] * (double)(2 * (r - delta) + 1);
+            const double w = (r - delta >= 0) ? v : 0.0;   // (a negative factor times 0.0 would store -0.0)
+            M[row - delta] = w;
+            if (bb) bb[row - delta] = w;
+        }
+    }
+}
+
+cudaError_t launch_band_writer(const BandWriterParams &P, cudaStream_t st)
+{
+    if (P.nmat <= 0) return cudaSuccess;
+    dim3 grid((unsigned)(P.lcut / WT + 1), (unsigned)((P.lmax + WT) / WT), (unsigned)P.nmat);
+    band_writer_kernel<<<grid, dim3(WT, WROWS, 1), 0, st>>>(P);
     return cudaGetLastError();
 }
 
