@@ -30,7 +30,10 @@ constexpr int SWEEP_THREADS = 32;
 #define TJ_R_POL 12
 #endif
 constexpr int R_POL = TJ_R_POL;           // pairs per thread, fused TT+TE+EE(+EB) sweep, dense storage
-constexpr int R_POL_BAND = 8;       // same, band-limited (short sweeps)
+#ifndef TJ_R_BAND
+#define TJ_R_BAND 8
+#endif
+constexpr int R_POL_BAND = TJ_R_BAND;       // same, band-limited (short sweeps)
 constexpr int R_TT = 16;            // pairs per thread, TT-only sweep (short sweeps)
 constexpr int R_TT_BAND = 16;       // same, band-limited
 constexpr int R_TT_LONG = 32;       // same, dense sweeps at lmax >= LMAX_LONG (measured at lmax = 10^4: 24.9 -> 22.8 ms)

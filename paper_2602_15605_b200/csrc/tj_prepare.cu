@@ -25,7 +25,8 @@ prepare_kernel(const double *__restrict__ Wtt, const double *__restrict__ Wtp, c
                int *tile_start, int lmax, int l3max_eff, int R, int banded, int row_lo, int row_hi)
 {
     const double inv4pi = 0.079577471545947667884441881686257181;  // 1/(4 pi)
-    const int lo = -GUARD_LO, hi = nl_alloc - GUARD_LO;
+    // band-limited calls (diagonal tiling) never read beyond l3max + 2 (R + TS) + 64 < l3max + GUARD_HI
+    const int lo = -GUARD_LO, hi = banded ? min(nl_alloc - GUARD_LO, l3max_eff + GUARD_HI) : nl_alloc - GUARD_LO;
     for (int l = lo + (int)(blockIdx.x * PREP_THREADS + threadIdx.x); l < hi; l += (int)(gridDim.x * PREP_THREADS)) {
         const bool in = (l >= 0 && l < nW && l <= l3max_eff);
         const double f = (2.0 * (double)l + 1.0) * inv4pi;
@@ -36,7 +37,7 @@ prepare_kernel(const double *__restrict__ Wtt, const double *__restrict__ Wtp, c
         wA[l] = make_double2((in && Wtt) ? f * Wtt[l] : 0.0, (in && Wtp) ? f * Wtp[l] : 0.0);
         wB[l] = make_double2((in && Wpp) ? f * Wpp[l] : 0.0, u3[l]);
     }
-    if (blockIdx.x != 0) return;
+    if (blockIdx.x != 0 || banded) return;   // the diagonal tiling decodes its tiles in closed form
 
     // ---- tile schedule: exclusive prefix over bands in descending order ----
     __shared__ int part[PREP_THREADS];
@@ -66,7 +67,8 @@ cudaError_t launch_prepare(const Tables &T, const double *d_Wtt, const double *d
                            double *wtt, double *wtp, double *wpp, double *wA, double *wB, int *tile_start, int R,
                            int l3max_eff, bool banded, int row_lo, int row_hi, cudaStream_t st)
 {
-    int nb = (T.nl_alloc + PREP_THREADS - 1) / PREP_THREADS;
+    const int nl = banded ? min(T.nl_alloc, GUARD_LO + l3max_eff + GUARD_HI) : T.nl_alloc;
+    int nb = (nl + PREP_THREADS - 1) / PREP_THREADS;
     if (nb > 64) nb = 64;
     prepare_kernel<<<nb, PREP_THREADS, 0, st>>>(d_Wtt, d_Wtp, d_Wpp, nW, wtt, wtp, wpp, (double2 *)wA, (double2 *)wB,
                                                  T.u3, T.nl_alloc, tile_start,

@@ -47,6 +47,8 @@
 // Bulk copies need 16-byte aligned source, destination and size; table slices start at any double, so a slice
 // whose first index is odd is fetched from the even index below it and the consumers add that parity `e` to
 // their offsets.  Stages advance by TS (even), so `e` is fixed per array for the whole walk.
+#include <type_traits>
+
 #include "tj_internal.cuh"
 
 namespace tj {
@@ -66,6 +68,9 @@ namespace {
 constexpr int TS_DENSE_LONG = TJ_TS_LONG, TS_DENSE_SHORT = TJ_TS_SHORT;
 #ifndef TJ_TS_BAND
 #define TJ_TS_BAND 64
+#endif
+#ifndef TJ_MINB_BAND
+#define TJ_MINB_BAND 3
 #endif
 constexpr int NBUF = 2;   // buffers per warp
 constexpr int PAD = 2;    // doubles in front of each slice: the software-pipelined read of "step TS" lands here
@@ -152,7 +157,7 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB * (128 / SWEEP_THREADS)) s
     extern __shared__ __align__(128) unsigned char smem_raw[];
     constexpr int NWARP = SWEEP_THREADS / 32;
 
-    static_assert(!DIAG || (SWEEP_THREADS == 32 && NW == 1 && SPIN == 2 && !ROWS), "diagonal tiling: one warp, one window set");
+    static_assert(!DIAG || (SWEEP_THREADS == 32 && NW == 1 && SPIN == 2 && !ROWS && !PIPE), "diagonal tiling: one warp, one window set, undeferred accumulation");
     const int lane = (int)(threadIdx.x & 31), warp = SWEEP_THREADS == 32 ? 0 : (int)(threadIdx.x >> 5);   // 0: keeps the warp's addresses CTA-uniform
     int a, cw;   // lane 0's first row and column
     if (DIAG) {
@@ -201,10 +206,21 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB * (128 / SWEEP_THREADS)) s
     // pair the row-ring loads too: those go into fixed ring registers and a paired load costs two register moves.
     // Diagonal tiling: lane j starts j steps after lane 0, so lane 0 may start below 0 (the guard band of g[t] adds
     // exact zeros there) but not below -32: then every lane starts at or below its own first step max(0, .).
-    tbo = DIAG ? max((tbo + 1) >> 1, -32) & P.even_mask : tbo > 0 ? ((tbo + 1) >> 1) & P.even_mask : 0;
+    // Then the first step moves further down so that the walk is whole blocks of R steps ENDING at the last step
+    // (leading steps have l3 > l3max, where the prefolded windows are 0): in the last block pair i is live in step
+    // u iff i >= u (even: t = a+u <= l1 = a+i; odd: t = a-1+u <= l1-1), and it runs in triangular form (below).
     int tbe = sw - P.l3max;        // even: l3 = s-2t   <= l3max
-    tbe = DIAG ? max((tbe + 1) >> 1, -32) & P.even_mask : tbe > 0 ? ((tbe + 1) >> 1) & P.even_mask : 0;
-    const int nso = (kEB && tbo <= t_end) ? (t_end - tbo + TS) / TS : 0;
+    const int t_end_o = DIAG ? t_end - 1 : t_end;   // odd branch: its last step is l1-1
+    if (DIAG) {
+        tbo = max((tbo + 1) >> 1, -32);
+        tbo = t_end_o + 1 - R * ((t_end_o - tbo + R) / R);
+        tbe = max((tbe + 1) >> 1, -32);
+        tbe = t_end + 1 - R * ((t_end - tbe + R) / R);
+    } else {
+        tbo = tbo > 0 ? ((tbo + 1) >> 1) & P.even_mask : 0;
+        tbe = tbe > 0 ? ((tbe + 1) >> 1) & P.even_mask : 0;
+    }
+    const int nso = (kEB && tbo <= t_end_o) ? (t_end_o - tbo + TS) / TS : 0;
     const int nse = (kEven && tbe <= t_end) ? (t_end - tbe + TS) / TS : 0;
     const int ntot = nso + nse;
 
@@ -295,7 +311,7 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB * (128 / SWEEP_THREADS)) s
             const int oh = L::OH + PAD + ((sw - tl0) & 1) + (TS - 1) + lane;
             for (int k = 0; k < nso; ++k, ++q) {
                 // blocks of R steps this stage really has (the last stage is cut at the band's last step)
-                const int nblk = min(TS / R, (t_end - (tbo + k * TS) + R) / R);
+                const int nblk = min(TS / R, (t_end_o - (tbo + k * TS) + R) / R);
                 const int b = q % NBUF;
                 mbar_wait(bar_s + 8u * b, (uint32_t)((q / NBUF) & 1));
                 const double *sb = wbuf + b * L::BUFD;
@@ -312,10 +328,12 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB * (128 / SWEEP_THREADS)) s
 #pragma unroll
                     for (int w = 1; w < NW; ++w) xw[w] = pB[w * L::CW].x;
                 }
-#pragma unroll 1
-                for (int blk = 0; blk < nblk; ++blk) {
+                // one block of R steps; TRI: the last block of the walk (diagonal tiling), pairs i < u are finished
+                auto block = [&](auto tri) {
+                    constexpr bool TRI = decltype(tri)::value;
 #pragma unroll
                     for (int u = 0; u < R; ++u) {
+                        const int i0 = TRI ? u : 0;
                         wa[(R - u) % R] = xa;
                         wb[(R + 1 - u) % R] = xb;
                         const double hg = __dmul_rn(xh, xg);
@@ -338,22 +356,27 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB * (128 / SWEEP_THREADS)) s
                         }
                         double r[R], e[R];
 #pragma unroll
-                        for (int i = 0; i < R; ++i) r[i] = __dmul_rn(wa[(i - u + R) % R], wb[(2 * R - i - u) % R]);
+                        for (int i = i0; i < R; ++i) r[i] = __dmul_rn(wa[(i - u + R) % R], wb[(2 * R - i - u) % R]);
                         if (SPIN == 2) {
 #pragma unroll
-                            for (int i = 0; i < R; ++i) e[i] = __dsub_rn(c3, c12[i]);
+                            for (int i = i0; i < R; ++i) e[i] = __dsub_rn(c3, c12[i]);
 #pragma unroll
-                            for (int i = 0; i < R; ++i) r[i] = __dmul_rn(r[i], e[i]);
+                            for (int i = i0; i < R; ++i) r[i] = __dmul_rn(r[i], e[i]);
 #pragma unroll
-                            for (int i = 0; i < R; ++i) r[i] = __dmul_rn(r[i], e[i]);
+                            for (int i = i0; i < R; ++i) r[i] = __dmul_rn(r[i], e[i]);
                         }
 #pragma unroll
                         for (int w = 0; w < NW; ++w)
 #pragma unroll
-                            for (int i = 0; i < R; ++i) acc[w][i] = __fma_rn(r[i], q3[w], acc[w][i]);
+                            for (int i = i0; i < R; ++i) acc[w][i] = __fma_rn(r[i], q3[w], acc[w][i]);
                     }
                     pa -= R; pb -= R; ph -= R; pg += R; pB -= 2 * R;
-                }
+                };
+                const bool tri_last = DIAG && k == nso - 1;
+                const int nfull = tri_last ? nblk - 1 : nblk;
+#pragma unroll 1
+                for (int blk = 0; blk < nfull; ++blk) block(std::false_type{});
+                if constexpr (DIAG) { if (tri_last) block(std::true_type{}); }
                 __syncwarp();
                 if (lane == 0 && q + NBUF < ntot) issue(q + NBUF);
             }
@@ -449,10 +472,11 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB * (128 / SWEEP_THREADS)) s
 #pragma unroll
                 for (int w = 0; w < NW; ++w) { xtt[w] = 0.0; xtp[w] = 0.0; xpp[w] = 0.0; }
                 load_w(0);
-#pragma unroll 1
-                for (int blk = 0; blk < nblk; ++blk) {
+                auto block = [&](auto tri) {   // as in the odd branch
+                    constexpr bool TRI = decltype(tri)::value;
 #pragma unroll
                     for (int u = 0; u < R; ++u) {
+                        const int i0 = TRI ? u : 0;
                         wa[(R - u) % R] = xa;
                         wb[(R + 1 - u) % R] = xb;
                         const double hg = __dmul_rn(xh, xg);
@@ -490,25 +514,25 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB * (128 / SWEEP_THREADS)) s
                         }
                         double r[R], A2[kA2 ? R : 1];
 #pragma unroll
-                        for (int i = 0; i < R; ++i) r[i] = __dmul_rn(wa[(i - u + R) % R], wb[(2 * R - i - u) % R]);
+                        for (int i = i0; i < R; ++i) r[i] = __dmul_rn(wa[(i - u + R) % R], wb[(2 * R - i - u) % R]);
                         if (kTT) {
 #pragma unroll
                             for (int w = 0; w < NW; ++w)
 #pragma unroll
-                                for (int i = 0; i < R; ++i) att[w][i] = __fma_rn(r[i], q0[w], att[w][i]);
+                                for (int i = i0; i < R; ++i) att[w][i] = __fma_rn(r[i], q0[w], att[w][i]);
                         }
                         if (kA2) {
 #pragma unroll
-                            for (int i = 0; i < R; ++i) A2[i] = __dsub_rn(c3, c12[i]);
+                            for (int i = i0; i < R; ++i) A2[i] = __dsub_rn(c3, c12[i]);
                             if (SPIN == 2) {
 #pragma unroll
-                                for (int i = 0; i < R; ++i) A2[i] = __fma_rn(A2[i], A2[i], -kk[i]);
+                                for (int i = i0; i < R; ++i) A2[i] = __fma_rn(A2[i], A2[i], -kk[i]);
                             }
 #pragma unroll
-                            for (int i = 0; i < R; ++i) rA[i] = __dmul_rn(r[i], A2[i]);
+                            for (int i = i0; i < R; ++i) rA[i] = __dmul_rn(r[i], A2[i]);
                             if (kEE) {
 #pragma unroll
-                                for (int i = 0; i < R; ++i) rAA[i] = __dmul_rn(rA[i], A2[i]);
+                                for (int i = i0; i < R; ++i) rAA[i] = __dmul_rn(rA[i], A2[i]);
                             }
                         }
                         if (!PIPE) {
@@ -516,18 +540,23 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB * (128 / SWEEP_THREADS)) s
                         for (int w = 0; w < NW; ++w) {
                             if (kTE) {
 #pragma unroll
-                                for (int i = 0; i < R; ++i) ate[w][i] = __fma_rn(rA[i], q1[w], ate[w][i]);
+                                for (int i = i0; i < R; ++i) ate[w][i] = __fma_rn(rA[i], q1[w], ate[w][i]);
                             }
                             if (kEE) {
 #pragma unroll
-                                for (int i = 0; i < R; ++i) aee[w][i] = __fma_rn(rAA[i], q2[w], aee[w][i]);
+                                for (int i = i0; i < R; ++i) aee[w][i] = __fma_rn(rAA[i], q2[w], aee[w][i]);
                             }
                         }
                         }
                     }
                     pa -= R; pb -= R; ph -= R; pg += R;
                     pwtt -= 2 * R; pA -= 2 * R; pB -= 2 * R;
-                }
+                };
+                const bool tri_last = DIAG && k == nse - 1;
+                const int nfull = tri_last ? nblk - 1 : nblk;
+#pragma unroll 1
+                for (int blk = 0; blk < nfull; ++blk) block(std::false_type{});
+                if constexpr (DIAG) { if (tri_last) block(std::true_type{}); }
                 __syncwarp();
                 if (lane == 0 && q + NBUF < ntot) issue(q + NBUF);
             }
@@ -635,11 +664,11 @@ cudaError_t launch_sweep(const SweepParams &P, int mask, int nw, int spin, int t
                           : (P.lmax >= LMAX_LONG ? launch_one<R_TT_LONG, M_TT, 64, 2, false>(P, total_tiles, st)
                                                  : launch_one<R_TT, M_TT, 48, 3, false>(P, total_tiles, st));
         case POL:
-            return banded ? launch_one<R_POL_BAND, POL, TJ_TS_BAND, 3, false, 1, 2, false, true>(P, total_tiles, st)
+            return banded ? launch_one<R_POL_BAND, POL, TJ_TS_BAND, TJ_MINB_BAND, false, 1, 2, false, true>(P, total_tiles, st)
                           : (P.lmax >= LMAX_LONG ? launch_one<R_POL, POL, TS_DENSE_LONG, TJ_MINB_POL, TJ_PIPE>(P, total_tiles, st)
                                                         : launch_one<R_POL, POL, TS_DENSE_SHORT, TJ_MINB_POL, TJ_PIPE>(P, total_tiles, st));
         case ALL:
-            return banded ? launch_one<R_POL_BAND, ALL, TJ_TS_BAND, 3, false, 1, 2, false, true>(P, total_tiles, st)
+            return banded ? launch_one<R_POL_BAND, ALL, TJ_TS_BAND, TJ_MINB_BAND, false, 1, 2, false, true>(P, total_tiles, st)
                           : (P.lmax >= LMAX_LONG ? launch_one<R_POL, ALL, TS_DENSE_LONG, TJ_MINB_POL, TJ_PIPE>(P, total_tiles, st)
                                                         : launch_one<R_POL, ALL, TS_DENSE_SHORT, TJ_MINB_POL, TJ_PIPE>(P, total_tiles, st));
         default: return cudaErrorInvalidValue;
