@@ -172,10 +172,13 @@ int tj_coupling_host(const tj_tables *tables, int band, int nW_or_lcut,
 int tj_l3_range(int l1, int l2, int l3max, int parity, int *l3_lo, int *l3_hi, int *nterms);
 
 /*
- * tj_sweep_counts -- the number of l3 terms the sweep kernel evaluates for one pair as the KERNEL
- * walks them (first/last step index t of the even and odd branch), so tests can check the
- * kernel's loop bounds against tj_l3_range / the oracle bit-exactly.  Host-side.
- *   even: l3 = l1+l2-2t, t = *te_lo..*te_hi;   odd: l3 = l1+l2-2t-1, t = *to_lo..*to_hi.
+ * tj_sweep_counts -- HOST-side closed form of the step indices t that carry the l3 terms of one pair:
+ *   even J: l3 = l1+l2-2t, t = *te_lo..*te_hi;   odd J: l3 = l1+l2-2t-1, t = *to_lo..*to_hi
+ * (l3 advances in steps of 2 from |l1-l2|; it stops at l3max).  It restates
+ * tj_l3_range in the sweep's step variable and is not what the kernels execute: a warp walks one common t range
+ * and the steps outside a pair's own range add exact zeros from the tables' guard bands.  The kernels' own
+ * bookkeeping is tested through their output (spike windows W = delta_{l,L} for every L: an entry is non-zero
+ * iff l3 = L is among the terms the kernel added; tests/test_gpu_parity.py).
  */
 int tj_sweep_counts(int l1, int l2, int l3max, int *te_lo, int *te_hi, int *to_lo, int *to_hi);
 
@@ -190,14 +193,23 @@ int tj_fp64_probe(int iters, void *cuda_stream, double *h_thread_instr_per_s);
  * Per-kernel timing for the roofline (bench.py): while enabled, every coupling call records CUDA events
  * on its stream around its three kernels.  tj_profile_get waits for the most recent call made by the
  * calling thread and returns the device time in milliseconds of  h_ms3[0] prepare (a2+a3),
- * h_ms3[1] sweep (a4+a5), h_ms3[2] writer (a6).  TJ_EINVAL if no profiled call was made on this thread.
+ * h_ms3[1] sweep (a4+a5), h_ms3[2] writer (a6); the single-launch path for small lmax reports its one kernel
+ * as the sweep.  tj_coupling_multi reports its last group of window sets.  TJ_EINVAL if the thread's most recent
+ * call was not profiled, or was tj_coupling_host / tj_coupling_literal (they record no per-kernel events).
  */
 int tj_profile_enable(int on);
 int tj_profile_get(double *h_ms3);
 
-/* Time of the last-enqueued work is the caller's to measure; this returns how many kernels the given
- * entry point launches per call (for bench.py's gpu_launches): which = 0 tt, 1 pol, 2 band. */
-int tj_launches_per_call(int which);
+/*
+ * tj_profile_last_sweep -- which sweep kernel the calling thread's most recent coupling call launched, so that a
+ * measurement can name the kernel it timed:  h_geo10 = { R (pairs per thread), block mask (1 TT | 2 TE | 4 EE | 8 EB),
+ * TS (steps per stage; 0 = the single-launch small_kernel), resident CTAs per SM / 4, deferred accumulation (0/1),
+ * window sets per sweep, spin, row-block form (0/1), diagonal band tiling (0/1), CTAs launched }.
+ * TJ_EINVAL before the first call.
+ * tj_profile_launches -- number of kernels the calling thread's calls have launched so far (callers take differences).
+ */
+int tj_profile_last_sweep(int *h_geo10);
+int tj_profile_launches(long long *h_count);
 
 const char *tj_strerror(int code);
 

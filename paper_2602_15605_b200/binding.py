@@ -20,7 +20,7 @@ SYMBOLS = (
     "tj_build_tables", "tj_free_tables", "tj_tables_info", "tj_tables_copy",
     "tj_coupling_tt", "tj_coupling_pol", "tj_coupling_band", "tj_coupling_multi", "tj_coupling_spin1", "tj_coupling_rows", "tj_coupling_literal", "tj_coupling_host",
     "tj_l3_range", "tj_sweep_counts", "tj_fp64_probe", "tj_profile_enable", "tj_profile_get",
-    "tj_launches_per_call", "tj_strerror",
+    "tj_profile_last_sweep", "tj_profile_launches", "tj_strerror",
 )
 
 
@@ -62,7 +62,8 @@ def load_library() -> ctypes.CDLL:
     L.tj_fp64_probe.argtypes = [ci, vp, dp]
     L.tj_profile_enable.argtypes = [ci]
     L.tj_profile_get.argtypes = [dp]
-    L.tj_launches_per_call.argtypes = [ci]
+    L.tj_profile_last_sweep.argtypes = [ip]
+    L.tj_profile_launches.argtypes = [ctypes.POINTER(ctypes.c_longlong)]
     L.tj_strerror.argtypes = [ci]
     L.tj_strerror.restype = ctypes.c_char_p
     for name in SYMBOLS:
@@ -306,8 +307,26 @@ def fp64_probe(iters=20000, stream=None):
     return v.value
 
 
-def launches_per_call(which: int) -> int:
-    return int(load_library().tj_launches_per_call(which))
+def profile_launches() -> int:
+    """Kernels this thread's calls have launched so far (take differences)."""
+    n = ctypes.c_longlong()
+    _check(load_library().tj_profile_launches(ctypes.byref(n)), "tj_profile_launches")
+    return int(n.value)
+
+
+def profile_last_sweep() -> dict:
+    """The sweep kernel this thread's most recent coupling call launched (include/tj.h)."""
+    g = (ctypes.c_int * 10)()
+    _check(load_library().tj_profile_last_sweep(g), "tj_profile_last_sweep")
+    keys = ("R", "mask", "TS", "minb", "pipe", "nw", "spin", "rows", "diag", "ctas")
+    d = dict(zip(keys, (int(x) for x in g)))
+    blocks = "|".join(n for b, n in ((1, "TT"), (2, "TE"), (4, "EE"), (8, "EB")) if d["mask"] & b)
+    if d["TS"] == 0:
+        d["name"] = "small_kernel<%s,R=%d> x %d CTAs of 128 threads" % (blocks, d["R"], d["ctas"])
+    else:
+        d["name"] = "sweep_tma_kernel<R=%d,%s,TS=%d,MINB=%d,PIPE=%d,NW=%d,SPIN=%d,ROWS=%d,DIAG=%d> x %d one-warp CTAs" % (
+            d["R"], blocks, d["TS"], d["minb"], d["pipe"], d["nw"], d["spin"], d["rows"], d["diag"], d["ctas"])
+    return d
 
 
 def profile_enable(on: bool) -> None:

@@ -88,6 +88,13 @@ struct Call {
     int dmax = 0;
 };
 
+// Dense single-window spin-2 calls at small lmax take the single-launch path (tj_small.cu): below LMAX_SMALL the
+// three launches and the scratch of the general path cost more than the arithmetic.
+bool use_small_path(const Tables &T, int lcut, int nw, int spin)
+{
+    return lcut < 0 && nw == 1 && spin == 2 && T.lmax <= LMAX_SMALL && small_smem_bytes(T.lmax, T.l3max) <= 200 * 1024;
+}
+
 // One coupling call on device pointers.  lcut < 0: dense (l3max = handle's); else banded with l3 <= lcut.
 int run_coupling(const tj_tables *tables, int lcut, const double *d_Wtt, const double *d_Wtp, const double *d_Wpp,
                  int nW, double *d_TT, double *d_TE, double *d_EE, double *d_BB, double *d_EB, cudaStream_t st, int nw = 1,
@@ -310,7 +317,7 @@ int tj_coupling_host(const tj_tables *tables, int band, int nW_or_lcut, const do
         int j = 0;
         for (int k = 0; k < 5; ++k)
             if (ho[k] && !(k == 3 && bb_from_ee)) dop[k] = dout + per * (size_t)(j++);
-        if (!band) {
+        if (!band && !use_small_path(T, -1, 1, 2)) {
             // dense: sweep, writer and the copies to the host pipelined by row chunks
             rc = run_coupling_rows_to_host(tables, dwp[0], dwp[1], dwp[2], nW, dop, ho, st);
         } else {
@@ -414,10 +421,20 @@ int tj_profile_get(double *h_ms3)
     return TJ_OK;
 }
 
-int tj_launches_per_call(int which)
+int tj_profile_last_sweep(int *h_geo10)
 {
-    // prepare + sweep + writer; the band call adds no kernel (its zero-fill is a memset)
-    return (which >= 0 && which <= 2) ? 3 : TJ_EINVAL;
+    if (!h_geo10) return TJ_EINVAL;
+    const SweepGeometry &G = g_last_sweep;
+    const int v[10] = {G.R, G.mask, G.TS, G.minb, G.pipe, G.nw, G.spin, G.rows, G.diag, G.tiles};
+    memcpy(h_geo10, v, sizeof(v));
+    return G.R > 0 ? TJ_OK : TJ_EINVAL;
+}
+
+int tj_profile_launches(long long *h_count)
+{
+    if (!h_count) return TJ_EINVAL;
+    *h_count = g_launch_count;
+    return TJ_OK;
 }
 
 }  // extern "C"
@@ -430,6 +447,7 @@ int coupling_begin(Call &C, const tj_tables *tables, int lcut, const double *d_W
                    cudaStream_t st, int nw = 1, int spin = 2, int row_lo = -1, int row_hi = -1)
 {
     const Tables &T = tables->T;
+    g_prof.valid = false;   // set again when this call has recorded all of its events
     C.T = &T;
     C.nw = nw;
     C.spin = spin;
@@ -447,7 +465,7 @@ int coupling_begin(Call &C, const tj_tables *tables, int lcut, const double *d_W
     if (!d_TE && !C.ee && !d_EB) C.mask = M_TT;
     else if (d_TT) C.mask = M_TT | M_TE | M_EE | M_EB;
     else C.mask = M_TE | M_EE | M_EB;
-    C.R = sweep_R(C.mask, C.banded, nw, T.lmax);
+    C.R = sweep_R(C.mask, C.banded, nw, T.lmax, row_lo >= 0, spin);
     C.l3max_eff = C.banded ? lcut : T.l3max;
     C.N = (long long)T.lmax + 1;
     C.rows = row_lo >= 0;
@@ -584,6 +602,17 @@ int run_coupling(const tj_tables *tables, int lcut, const double *d_Wtt, const d
                  int nW, double *d_TT, double *d_TE, double *d_EE, double *d_BB, double *d_EB, cudaStream_t st, int nw,
                  int spin)
 {
+    if (use_small_path(tables->T, lcut, nw, spin)) {
+        // single-launch path (tj_small.cu): no scratch, no tile list
+        if ((d_TT && !d_Wtt) || (d_TE && !d_Wtp) || ((d_EE || d_BB || d_EB) && !d_Wpp)) return TJ_EINVAL;
+        if (!d_TT && !d_TE && !d_EE && !d_BB && !d_EB) return TJ_EINVAL;
+        const int mask = (!d_TE && !d_EE && !d_BB && !d_EB) ? M_TT : (d_TT ? M_TT : 0) | M_TE | M_EE | M_EB;
+        g_prof.valid = false;
+        prof_record(0, st); prof_record(1, st); prof_record(2, st);
+        cudaError_t e = launch_small(tables->T, mask, d_Wtt, d_Wtp, d_Wpp, nW, d_TT, d_TE, d_EE, d_BB, d_EB, st);
+        prof_record(3, st); prof_record(4, st);
+        return e == cudaSuccess ? TJ_OK : cuda_fail(e, "coupling/small");
+    }
     Call C;
     int rc = coupling_begin(C, tables, lcut, d_Wtt, d_Wtp, d_Wpp, nW, d_TT, d_TE, d_EE, d_BB, d_EB, st, nw, spin);
     if (rc != TJ_OK) return rc;

@@ -33,10 +33,16 @@ constexpr int R_POL = TJ_R_POL;           // pairs per thread, fused TT+TE+EE(+E
 #ifndef TJ_R_BAND
 #define TJ_R_BAND 8
 #endif
+constexpr int R_POL_MID = 8;        // same at lmax < LMAX_MID: shorter sweeps, fewer tiles -- smaller tiles balance better (measured at lmax = 2000: 1.288 -> 1.230 ms per call)
+constexpr int LMAX_MID = 2600;
 constexpr int R_POL_BAND = TJ_R_BAND;       // same, band-limited (short sweeps)
 constexpr int R_TT = 16;            // pairs per thread, TT-only sweep (short sweeps)
 constexpr int R_TT_BAND = 16;       // same, band-limited
 constexpr int R_TT_LONG = 32;       // same, dense sweeps at lmax >= LMAX_LONG (measured at lmax = 10^4: 24.9 -> 22.8 ms)
+#ifndef TJ_LMAX_SMALL
+#define TJ_LMAX_SMALL 800
+#endif
+constexpr int LMAX_SMALL = TJ_LMAX_SMALL;   // up to here dense single-window calls take the single-launch path (tj_small.cu)
 constexpr int LMAX_LONG = 4096;     // from here on a dense sweep uses the long-sweep geometry (R_TT_LONG; 96-step stages)
 constexpr int R_MULTI2 = 8;         // pairs per thread, 2 window sets per sweep (tj_coupling_multi)
 constexpr int R_MULTI3 = 6;         // pairs per thread, 3 window sets per sweep
@@ -92,8 +98,10 @@ __host__ __device__ inline int diag_num_groups(int dmax, int R)
 __host__ __device__ inline int diag_num_blocks(int lmax, int R) { return (lmax + R + 31) / 32; }
 
 // the sweep instantiation a launch used (for the roofline label of bench.py, tj_profile_geometry)
-struct SweepGeometry { int R, mask, TS, minb, pipe, nw, spin, rows, diag, tiles; };
+struct SweepGeometry { int R, mask, TS, minb, pipe, nw, spin, rows, diag, tiles; };   // TS = 0: small_kernel (tj_small.cu)
 extern thread_local SweepGeometry g_last_sweep;
+// kernels launched by this thread's coupling calls since the library was loaded (tj_profile_launches)
+extern thread_local long long g_launch_count;
 
 struct Tables {
     int lmax, l3max, pmax;          // p-tables hold p = 0..pmax = 2*lmax+1
@@ -154,10 +162,14 @@ cudaError_t launch_prepare(const Tables &T, const double *d_Wtt, const double *d
                            int l3max_eff, bool banded, int row_lo, int row_hi, cudaStream_t st);
 // row-block outputs: M[r][c] *= (2c+1) for the nmat blocks in M (rows x (lmax+1) each), bb = copy of M[bb_src] or NULL
 cudaError_t launch_scale_rows(double *const M[4], int nmat, double *bb, int bb_src, long long rows, int lmax, cudaStream_t st);
-int sweep_R(int mask, bool banded, int nw, int lmax);   // pairs per thread (= rows per band) of the sweep that serves `mask` for nw window sets
+int sweep_R(int mask, bool banded, int nw, int lmax, bool rows, int spin);   // pairs per thread (= rows per band) of the sweep that serves `mask` for nw window sets
 cudaError_t launch_sweep(const SweepParams &P, int mask, int nw, int spin, int total_tiles, cudaStream_t st);
 cudaError_t launch_writer(const WriterParams &P, cudaStream_t st);
 cudaError_t launch_band_writer(const BandWriterParams &P, cudaStream_t st);
+// single-launch path for small lmax (tj_small.cu)
+size_t small_smem_bytes(int lmax, int l3max);
+cudaError_t launch_small(const Tables &T, int mask, const double *d_Wtt, const double *d_Wtp, const double *d_Wpp, int nW,
+                         double *TT, double *TE, double *EE, double *BB, double *EB, cudaStream_t st);
 cudaError_t launch_literal(const Tables &T, const double *wtt, const double *wpp, double *TT, double *EE, int l3max,
                            cudaStream_t st);   // paper-literal ablation kernel (tj_literal.cu)
 cudaError_t launch_fp64_probe(int iters, double *d_sink, int blocks, int threads, cudaStream_t st);

@@ -78,6 +78,7 @@ cudaError_t launch_literal(const Tables &T, const double *wtt, const double *wpp
     const int N = T.lmax + 1;
     dim3 grid((unsigned)((N + LIT_THREADS - 1) / LIT_THREADS), (unsigned)N, 1);
     literal_kernel<<<grid, LIT_THREADS, 0, st>>>(T.g, T.h, wtt, wpp, TT, EE, T.lmax, l3max);
+    ++g_launch_count;
     return cudaGetLastError();
 }
 

@@ -73,6 +73,7 @@ cudaError_t launch_prepare(const Tables &T, const double *d_Wtt, const double *d
     prepare_kernel<<<nb, PREP_THREADS, 0, st>>>(d_Wtt, d_Wtp, d_Wpp, nW, wtt, wtp, wpp, (double2 *)wA, (double2 *)wB,
                                                  T.u3, T.nl_alloc, tile_start,
                                                  T.lmax, l3max_eff, R, banded ? 1 : 0, row_lo, row_hi);
+    ++g_launch_count;
     return cudaGetLastError();
 }
 

@@ -612,12 +612,14 @@ cudaError_t launch_one(const SweepParams &P, int total_tiles, cudaStream_t st)
         if (e != cudaSuccess) return e;
     }
     sweep_tma_kernel<R, MASK, TS, MINB, PIPE, NW, SPIN, ROWS, DIAG><<<total_tiles, SWEEP_THREADS, smem, st>>>(P);
+    ++g_launch_count;
     return cudaGetLastError();
 }
 
 }  // namespace
 
 thread_local SweepGeometry g_last_sweep = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
+thread_local long long g_launch_count = 0;
 
 // Geometry per request: dense sweeps are long (up to lmax steps per pair), so the per-step
 // overhead (prefactors, table reads) is spread over R = 12 pairs at 2 CTAs/SM with stages of 96 (48) steps;
@@ -625,13 +627,14 @@ thread_local SweepGeometry g_last_sweep = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
 // Multi-window batching (nw window sets in one sweep): the geometric part of a term (r, A2, rA, rAA) is
 // computed once and each window set adds 3 FMAs (1 in the odd branch); the accumulators of nw sets take the
 // registers that R = 12 pairs use otherwise, hence R = 8 for nw = 2 and R = 6 for nw = 3.
-int sweep_R(int mask, bool banded, int nw, int lmax)
+int sweep_R(int mask, bool banded, int nw, int lmax, bool rows, int spin)
 {
     if (mask == M_TT && nw > 1) return R_TT_MULTI;
     if (nw == 2) return R_MULTI2;
     if (nw == 3) return R_MULTI3;
     if (mask == M_TT) return banded ? R_TT_BAND : lmax >= LMAX_LONG ? R_TT_LONG : R_TT;
-    return banded ? R_POL_BAND : R_POL;
+    if (banded) return R_POL_BAND;
+    return (!rows && spin == 2 && lmax < LMAX_MID) ? R_POL_MID : R_POL;
 }
 
 cudaError_t launch_sweep(const SweepParams &P, int mask, int nw, int spin, int total_tiles, cudaStream_t st)
@@ -665,12 +668,12 @@ cudaError_t launch_sweep(const SweepParams &P, int mask, int nw, int spin, int t
                                                  : launch_one<R_TT, M_TT, 48, 3, false>(P, total_tiles, st));
         case POL:
             return banded ? launch_one<R_POL_BAND, POL, TJ_TS_BAND, TJ_MINB_BAND, false, 1, 2, false, true>(P, total_tiles, st)
-                          : (P.lmax >= LMAX_LONG ? launch_one<R_POL, POL, TS_DENSE_LONG, TJ_MINB_POL, TJ_PIPE>(P, total_tiles, st)
-                                                        : launch_one<R_POL, POL, TS_DENSE_SHORT, TJ_MINB_POL, TJ_PIPE>(P, total_tiles, st));
+                          : (P.lmax >= LMAX_MID ? launch_one<R_POL, POL, TS_DENSE_LONG, TJ_MINB_POL, TJ_PIPE>(P, total_tiles, st)
+                                                       : launch_one<R_POL_MID, POL, TS_DENSE_LONG, 2, TJ_PIPE>(P, total_tiles, st));
         case ALL:
             return banded ? launch_one<R_POL_BAND, ALL, TJ_TS_BAND, TJ_MINB_BAND, false, 1, 2, false, true>(P, total_tiles, st)
-                          : (P.lmax >= LMAX_LONG ? launch_one<R_POL, ALL, TS_DENSE_LONG, TJ_MINB_POL, TJ_PIPE>(P, total_tiles, st)
-                                                        : launch_one<R_POL, ALL, TS_DENSE_SHORT, TJ_MINB_POL, TJ_PIPE>(P, total_tiles, st));
+                          : (P.lmax >= LMAX_MID ? launch_one<R_POL, ALL, TS_DENSE_LONG, TJ_MINB_POL, TJ_PIPE>(P, total_tiles, st)
+                                                       : launch_one<R_POL_MID, ALL, TS_DENSE_LONG, 2, TJ_PIPE>(P, total_tiles, st));
         default: return cudaErrorInvalidValue;
     }
 }

@@ -119,6 +119,7 @@ cudaError_t launch_scale_rows(double *const M[4], int nmat, double *bb, int bb_s
     long long nb = (total + 255) / 256;
     if (nb > 148 * 32) nb = 148 * 32;
     scale_rows_kernel<<<(unsigned)nb, 256, 0, st>>>(M[0], M[1], M[2], M[3], nmat, bb, bb_src, total, lmax + 1);
+    ++g_launch_count;
     return cudaGetLastError();
 }
 
@@ -170,6 +171,7 @@ cudaError_t launch_band_writer(const BandWriterParams &P, cudaStream_t st)
     if (P.nmat <= 0) return cudaSuccess;
     dim3 grid((unsigned)(P.lcut / WT + 1), (unsigned)((P.lmax + WT) / WT), (unsigned)P.nmat);
     band_writer_kernel<<<grid, dim3(WT, WROWS, 1), 0, st>>>(P);
+    ++g_launch_count;
     return cudaGetLastError();
 }
 
@@ -179,6 +181,7 @@ cudaError_t launch_writer(const WriterParams &P, cudaStream_t st)
     dim3 grid((unsigned)((P.I1 - P.I0) * (P.tile_band + 1)), 1, 1);
     dim3 block(WT, WROWS, 1);
     writer_kernel<<<grid, block, 0, st>>>(P);
+    ++g_launch_count;
     return cudaGetLastError();
 }
 

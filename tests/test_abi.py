@@ -36,7 +36,9 @@ def test_every_declared_symbol_is_exported(lib):
 def test_strerror(lib):
     assert lib.tj_strerror(0) == b"ok"
     assert b"invalid" in lib.tj_strerror(-1)
-    assert lib.tj_launches_per_call(1) == 3
+    n = ctypes.c_longlong(-1)
+    assert lib.tj_profile_launches(ctypes.byref(n)) == 0 and n.value >= 0
+    assert lib.tj_profile_launches(None) == binding.TJ_EINVAL
 
 
 def test_argument_errors_without_gpu(lib):
