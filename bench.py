@@ -44,6 +44,20 @@ def _peaks():
     return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "sm_max_mhz": 1965.0}, "fallback"
 
 
+def _traffic(workload, geo):
+    """DRAM bytes of one sweep launch for this workload from profiles/traffic.csv (written from ncu --set full
+    captures; columns: workload, kernel prefix, dram_read_bytes, dram_write_bytes, capture)."""
+    p = os.path.join(ROOT, "profiles", "traffic.csv")
+    if workload is None or not os.path.exists(p):
+        return None, None
+    import csv
+    with open(p) as fh:
+        for row in csv.DictReader(fh):
+            if row["workload"] == workload and geo["name"].startswith(row["kernel_prefix"]):
+                return float(row["dram_read_bytes"]) + float(row["dram_write_bytes"]), row["capture"]
+    return None, None
+
+
 class ClockSampler:
     """nvidia-smi sampling DURING the timed region (B200_PROFILING.md clocks line)."""
     Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
@@ -128,6 +142,42 @@ def time_oracle(wl, cfg, reps=1):
             "sample": what, "sample_terms": terms, "sample_seconds": best}
 
 
+def time_table_method(wl, cfg):
+    """The paper's own CPU design (bench_cpu/tablemethod.c: lookup tables, OpenMP dynamic over l1) beside the
+    Schulten-Gordon oracle on the same host cores and the same row sample, TT and EE separately -- the paper's
+    "6-25x over recursion-based pipelines" re-measured on this box."""
+    import numpy as np
+    import bench_cpu
+    import oracle
+    l1, l2, _, what = _oracle_sample(wl.lmax, cfg)
+    rows = np.unique(l1).astype(np.int32)
+    bench_cpu.lib()
+    oracle.lib()
+
+    def best(f, reps):
+        b = None
+        for _ in range(reps):
+            t0 = time.perf_counter()
+            f()
+            dt = time.perf_counter() - t0
+            b = dt if b is None else min(b, dt)
+        return b
+    t_tm_tt = best(lambda: bench_cpu.coupling_rows(wl.lmax, wl.l3max, wl.Wtt, None, rows), 2)
+    t_tm_ee = best(lambda: bench_cpu.coupling_rows(wl.lmax, wl.l3max, None, wl.Wpp, rows), 2)
+    t_or_tt = best(lambda: oracle.coupling_pairs(wl.l3max, wl.Wtt, None, None, l1, l2), 1)
+    t_or_ee = best(lambda: oracle.coupling_pairs(wl.l3max, None, None, wl.Wpp, l1, l2), 1)
+    # even-J terms of the sampled rows (what the table method evaluates per matrix)
+    lo = np.abs(l1.astype(np.int64) - l2)
+    hi = np.minimum(l1.astype(np.int64) + l2, wl.l3max)
+    terms_even = int(np.maximum((hi - lo) // 2 + 1, 0).sum())
+    return {"kind": "paper's table method on the host cores (bench_cpu/tablemethod.c)", "cores": bench_cpu.num_threads(),
+            "sample": what.replace("all blocks", "TT and EE separately"), "unit": UNIT,
+            "tt": {"table_method_s": t_tm_tt, "oracle_s": t_or_tt, "speedup": t_or_tt / t_tm_tt, "value": terms_even / t_tm_tt},
+            "ee": {"table_method_s": t_tm_ee, "oracle_s": t_or_ee, "speedup": t_or_ee / t_tm_ee, "value": terms_even / t_tm_ee},
+            "paper": "TT 25.3x, EE 6.7x over the S-G reference at lmax = 4722 on 8 Apple-M3 cores (PAPER.md:232-234); "
+                     "headline 6-25x (PAPER.md:17)"}
+
+
 def run_reference(args):
     """--impl reference: the oracle as it stands, on the host cores, on a bounded sample per step."""
     rank = int(os.environ.get("RANK", "0"))
@@ -175,6 +225,7 @@ def main():
                     help="also time tj_coupling_literal (the paper's per-pair Eq. 10 / Eq. 16 evaluation) on the same workload")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-cpu-table-method", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -257,10 +308,39 @@ def main():
             dist.barrier()
             torch.cuda.synchronize()
 
+    n0 = binding.profile_launches()
+    step()
+    launches_per_step = binding.profile_launches() - n0
     binding.profile_enable(True)
     for _ in range(max(args.warmup, 3)):
         step()
     sync_all()
+    geo = binding.profile_last_sweep()
+    # A step shorter than ~1 ms is launch-bound: the library's five profiling events per call and the Python side
+    # of the call would be a visible part of it.  Such a step is timed WITHOUT the profiling events and as the replay of
+    # a CUDA graph that holds ONE call (launch-bound inner loops belong in CUDA graphs); the per-kernel times then come
+    # from a separate profiled pass of the same steps, by direct calls, right after the timed region.
+    ws, we = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ws.record(); step(); we.record(); torch.cuda.synchronize()
+    est_ms = ws.elapsed_time(we)
+    profile_in_region = est_ms >= 1.0
+    use_graph = est_ms < 1.0 and dist is None
+    binding.profile_enable(profile_in_region)
+    graph = None
+    run = step
+    if use_graph:
+        gs = torch.cuda.Stream()
+        gs.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(gs):
+            step()
+            graph = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(graph, stream=gs):
+                step()
+        torch.cuda.current_stream().wait_stream(gs)
+        run = graph.replay
+        for _ in range(3):
+            run()
+        sync_all()
 
     sampler = ClockSampler(local_rank)
     sampler.start()
@@ -272,13 +352,21 @@ def main():
     for i in range(args.steps):
         flush.fill_(float(i))            # L2 flush between timed iterations (outside the event pair)
         ev[i][0].record()
-        step()
+        run()
         ev[i][1].record()
-        kern.append(binding.profile_get())   # waits for this step's kernels (per-kernel device times)
+        if profile_in_region:
+            kern.append(binding.profile_get())   # waits for this step's kernels (per-kernel device times)
     sync_all()
     t_wall = time.perf_counter() - t_wall0
     clocks = sampler.stop()
     step_ms = [a.elapsed_time(b) for a, b in ev]
+    if not profile_in_region:
+        binding.profile_enable(True)
+        for i in range(args.steps):
+            flush.fill_(float(i))
+            step()
+            kern.append(binding.profile_get())
+        sync_all()
     total_ms = float(sum(step_ms))
     total_ms = shard.max_over_ranks(total_ms, dist, "cuda")
     # split rows: the job is ONE matrix set (its terms counted once); else every rank does `terms`
@@ -312,26 +400,42 @@ def main():
         alg_instr *= last
         alg_flops *= last
     peaks, peak_kind = _peaks()
+    traffic, traffic_src = _traffic(wl.name if nwin == 1 and not split else None, geo)
     sm_max = float(clocks.get("sm_max_mhz") or peaks.get("sm_max_mhz", 1965.0))
     peak_instr = SM_COUNT * FP64_LANES_PER_SM * sm_max * 1e6          # thread-instr/s at max boost
     achieved = alg_instr / (sweep_ms * 1e-3)
-    probe = binding.fp64_probe(40000)
+    # measured DFMA rate: a register-resident chain kernel on every SM for >= 1 s, clocks sampled
+    it = 2000000
+    rate = binding.fp64_probe(it)
+    it = int(min(2.0e9, 1.15 * it * rate / (16.0 * it * SM_COUNT * 4 * 256)))   # iterations for ~1.15 s at that rate
+    psampler = ClockSampler(local_rank)
+    psampler.start()
+    time.sleep(0.2)
+    tp0 = time.perf_counter()
+    probe = binding.fp64_probe(it)
+    probe_s = time.perf_counter() - tp0
+    probe_clocks = psampler.stop()
     bytes_out = len(blocks) * N * width * 8
     nmirror = len(blocks) - (1 if "BB" in blocks else 0)
     writer_bytes = int(nmirror * 1.5 * N * width * 8 + (N * width * 8 if "BB" in blocks else 0))
     roofline = {
-        "bound": "alu", "kernel": "sweep_tma_kernel<R=6,TT|TE|EE|EB,TS=36,PIPE,NW=3> (last group of the call)" if nwin > 1 else ("sweep_tma_kernel<R=8,TS=32>" if wl.band else "sweep_tma_kernel<R=12,TT|TE|EE|EB,TS=48,PIPE>") if wl.pol else "sweep_tma_kernel<R=16,TT>",
+        # the instantiation the library really launched (tj_profile_last_sweep), not a label typed here
+        "bound": "alu", "kernel": geo["name"] + (" (last group of the call)" if nwin > 1 else ""),
         "achieved": achieved / 1e12, "peak": peak_instr / 1e12, "unit": "T FP64 thread-instr/s",
         "frac": achieved / peak_instr,
-        # dram__bytes_read.sum + dram__bytes_write.sum of one sweep launch, from the ncu --set full capture
-        # profiles/r1_ncu_full_cfg3.md (config 3 only; other configs: not captured)
-        "traffic": 1.571e9 if (args.config == 3 and wl.pol) else None,
+        # dram__bytes_read.sum + dram__bytes_write.sum of one launch of this kernel, from the committed ncu --set full
+        # summaries (profiles/traffic.csv names the capture each row comes from); None if this workload has no capture
+        "traffic": traffic, "traffic_source": traffic_src,
         "peak_source": "derived: %d SMs x %d FP64 lanes/clk x %.0f MHz (DESIGN.md 6; MEASURED_PEAKS.json has no FP64 entry)"
                        % (SM_COUNT, FP64_LANES_PER_SM, sm_max),
         "algorithmic_instr_per_launch": alg_instr, "algorithmic_flops_per_launch": alg_flops,
         "achieved_tflops": alg_flops / (sweep_ms * 1e-3) / 1e12,
         "measured_dfma_peak": probe / 1e12, "frac_of_measured_dfma": achieved / probe,
+        "dfma_probe": {"seconds": probe_s, "iterations": it, "sm_mhz": probe_clocks.get("sm_mhz"),
+                       "reasons": probe_clocks.get("reasons"), "power_w_max": probe_clocks.get("power_w_max")},
         "kernel_ms": {"prepare": prep_ms, "sweep": sweep_ms, "writer": writer_ms},
+        "kernel_ms_source": "library CUDA events inside the timed region" if profile_in_region
+                            else "library CUDA events in a separate profiled pass of the same steps after the timed region",
         "sweep_share_of_step": sweep_ms / (total_ms / args.steps) if world == 1 else None,
         # writer: per mirrored block reads the upper triangle (N^2/2) and writes N^2; BB is one more N^2 write
         "writer": {"bound": "hbm", "achieved": writer_bytes / (writer_ms * 1e-3) / 1e9, "peak": peaks.get("hbm_gbs"),
@@ -380,6 +484,9 @@ def main():
     cpu_baseline = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline and not wl.band:
         cpu_baseline = time_oracle(wl, args.config)
+    cpu_table_method = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline and not args.no_cpu_table_method and not wl.band and wl.pol:
+        cpu_table_method = time_table_method(wl, args.config)
 
     if rank == 0:
         line = {
@@ -392,10 +499,11 @@ def main():
                        "l2": "512 MB flush written between timed steps; each step also writes %.1f GB of output" % (bytes_out / 1e9),
                        "parallelism": ("one matrix set cut into %d row blocks (tj_coupling_rows), rank 0 rows [%d,%d)" % (world, row_lo, row_hi))
                        if split else ("1 problem per GPU" if world > 1 else "single GPU")},
-            "roofline": roofline, "cpu_baseline": cpu_baseline, "e2e": e2e, "ablation": ablation,
-            # per window set one prepare + one writer launch, per group of sets (3, or 2 + 2 for a remainder of 4) one sweep
-            "gpu_launches": (2 * nwin + ngroups) * args.steps if nwin > 1
-            else binding.launches_per_call(1) * args.steps,
+            "roofline": roofline, "cpu_baseline": cpu_baseline, "cpu_table_method": cpu_table_method, "e2e": e2e,
+            "ablation": ablation,
+            # kernels of libtj launched inside the timed region, counted by the library (tj_profile_launches)
+            "gpu_launches": launches_per_step * args.steps, "gpu_launches_per_step": launches_per_step,
+            "launch": "replay of a CUDA graph holding one call" if use_graph else "direct calls",
             "clocks": clocks, "wall_s_timed_region": t_wall, "step_ms": step_ms,
             "context": {"paper_A100_TT_lmax1e4_s": 0.63, "paper_A100_EE_lmax1e4_s": 3.2,
                         "note": "paper numbers (PAPER.md:242) are another machine's: context, not the target"},

@@ -23,9 +23,9 @@ constexpr int SM_THREADS = 128;
 // per call, all five blocks: lmax 256: 20.9 us with R = 2, 24.9 with R = 4; lmax 640: 124 vs 108 us).
 constexpr int SM_LMAX_R2 = 400;
 constexpr int SM_U = 4;      // steps per block: operands of U steps are loaded before their arithmetic starts
-constexpr int SM_GL = 16;    // zero doubles below index 0 of every shared table (indices reach -2(R-1)-U, windows -2(R+U))
+constexpr int SM_GL = 32;    // zero doubles below index 0 of every shared table (indices reach -2(R-1)-2U, windows -2(R+2U))
 constexpr int SM_GH = 16;    // and above the last entry (h[s-t] reaches pmax + R/2)
-static_assert(2 * (4 + SM_U) <= SM_GL, "low guard");
+static_assert(2 * (4 + 2 * SM_U) <= SM_GL, "low guard");
 
 struct SmallParams {
     const double *g, *ginv, *h, *gA, *gB, *isd;   // the handle's tables (index 0)
@@ -42,6 +42,7 @@ __global__ void __launch_bounds__(SM_THREADS) small_kernel(const __grid_constant
 {
     constexpr bool kTT = (MASK & M_TT) != 0, kPol = (MASK & (M_TE | M_EE | M_EB)) != 0;
     constexpr int U = SM_U;
+    constexpr bool SWP = !kPol;    // TT alone: the products of block k+1 are formed while the chains of block k run
     extern __shared__ __align__(16) double sm[];
     const int np = SM_GL + P.pmax + 1 + SM_GH, nl = SM_GL + P.l3max + 1 + SM_GH;
     const bool odd = kPol && blockIdx.z == 1;
@@ -119,11 +120,54 @@ __global__ void __launch_bounds__(SM_THREADS) small_kernel(const __grid_constant
     for (int i = 0; i < R; ++i) { acc0[i] = 0.0; acc1[i] = 0.0; acc2[i] = 0.0; }
 
     // l3 = s-2t-par <= l3max.  Steps run in blocks of U: every operand of a block is loaded before its arithmetic
-    // starts (one warp per scheduler is the common case here: latency, not issue, is what counts), and the walk is
-    // extended past t_end to whole blocks -- there the ring factors are the zero guards and add exact zeros.
+    // starts, and the arithmetic is operation-major over the U x R terms of the block (every level is U*R independent
+    // instructions): one warp per scheduler is the common case here, and a dependent FP64 operation costs ~30 cycles,
+    // so latency, not issue, is what counts.  Only the accumulations are ordered (in t).  With SWP (TT alone) the
+    // products of block k+1 are formed while the accumulation chains of block k run (software pipelining by one
+    // block: lmax = 256 10.6 -> 8.3 us; for the polarised blocks the second set of products costs more registers
+    // than the overlap gains).  The walk is extended past t_end to whole blocks -- there the ring factors are the
+    // zero guards and add exact zeros -- and SWP prepares one block more, which is never accumulated.
     const int par = odd ? 1 : 0;
     int tb = s - par - P.l3max;
     tb = tb > 0 ? (tb + 1) >> 1 : 0;
+    if (SWP) {   // TT alone: two sets of block products (q0 = W' h g[t], r) alternate
+        struct Prod { double q0[U], r[U][R]; };
+        auto prepare = [&](int t0, Prod &B) {
+            double vh[U], vg[U], vb[U][R];
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                const int t = t0 + u;
+                vh[u] = sc[s - t];
+                vg[u] = sb[t];
+                B.q0[u] = sw0[s - 2 * t];
+#pragma unroll
+                for (int i = 0; i < R; ++i) { B.r[u][i] = sa[a + i - t]; vb[u][i] = sa[c - i - t]; }
+            }
+#pragma unroll
+            for (int u = 0; u < U; ++u) vh[u] = __dmul_rn(vh[u], vg[u]);                      // hg
+#pragma unroll
+            for (int u = 0; u < U; ++u) B.q0[u] = __dmul_rn(B.q0[u], vh[u]);                  // q0
+#pragma unroll
+            for (int u = 0; u < U; ++u)
+#pragma unroll
+                for (int i = 0; i < R; ++i) B.r[u][i] = __dmul_rn(B.r[u][i], vb[u][i]);       // r
+        };
+        auto accumulate = [&](const Prod &B) {
+#pragma unroll
+            for (int u = 0; u < U; ++u)
+#pragma unroll
+                for (int i = 0; i < R; ++i) acc0[i] = __fma_rn(B.r[u][i], B.q0[u], acc0[i]);
+        };
+        Prod A, B;
+        prepare(tb, A);
+        for (int t0 = tb; t0 <= t_end; t0 += 2 * U) {
+            prepare(t0 + U, B);
+            accumulate(A);
+            if (t0 + U > t_end) break;
+            prepare(t0 + 2 * U, A);
+            accumulate(B);
+        }
+    } else {
     for (int t0 = tb; t0 <= t_end; t0 += U) {
         double vh[U], vg[U], w0[U], w1[U], w2[U], c3[U], r[U][R], vb[U][R];
 #pragma unroll
@@ -138,8 +182,6 @@ __global__ void __launch_bounds__(SM_THREADS) small_kernel(const __grid_constant
 #pragma unroll
             for (int i = 0; i < R; ++i) { r[u][i] = sa[a + i - t]; vb[u][i] = sa[c - i - t]; }
         }
-        // operation-major over the U x R terms of the block: every level is U*R independent instructions, so the
-        // latency of one level hides behind the issue of the next; only the accumulations are ordered (in t)
 #pragma unroll
         for (int u = 0; u < U; ++u) vh[u] = __dmul_rn(vh[u], vg[u]);                      // hg
 #pragma unroll
@@ -204,6 +246,7 @@ __global__ void __launch_bounds__(SM_THREADS) small_kernel(const __grid_constant
                     for (int i = 0; i < R; ++i) acc2[i] = __fma_rn(r[u][i], w2[u], acc2[i]);
             }
         }
+    }
     }
 
     // ---- scale, mirror, store (steps a5 + a6) ----

@@ -47,8 +47,6 @@
 // Bulk copies need 16-byte aligned source, destination and size; table slices start at any double, so a slice
 // whose first index is odd is fetched from the even index below it and the consumers add that parity `e` to
 // their offsets.  Stages advance by TS (even), so `e` is fixed per array for the whole walk.
-#include <type_traits>
-
 #include "tj_internal.cuh"
 
 namespace tj {
@@ -106,11 +104,12 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t
 }
 
 // capacities (doubles, all even) of the slices inside one stage buffer
-template <int TS, int NW, bool PK> struct Lay {
+template <int TS, int NW, bool PK, bool DIAG> struct Lay {
     static constexpr int CA = PAD + TS + 2;            // row ring / step factor
     static constexpr int CB = PAD + TS + 32 + 2;       // column ring / h
     static constexpr int CW = PAD + 2 * TS + 32 + 2;   // windows, u3
-    static constexpr int OA = 0, OG = OA + CA, OB = OG + CB, OH = OB + CB;   // OG: CB doubles (the diagonal tiling reads g[t] per lane)
+    // the diagonal tiling reads the step factor per lane (TS+31 values) and the column ring as a broadcast
+    static constexpr int OA = 0, OG = OA + CA, OB = OG + (DIAG ? CB : CA), OH = OB + (DIAG ? CA : CB);
     static constexpr int OW0 = OH + CB;                // TT-only sweep: the plain W'_TT slices, one per window set
     // polarised sweeps read the windows as pairs (prepare_kernel): (W'_TT, W'_TP)[l] and (W'_PP, u_l)[l], one array
     // of 2*CW doubles per window set each, in the same region (the TT-only sweep keeps the plain W'_TT slot OW0)
@@ -144,7 +143,7 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB * (128 / SWEEP_THREADS)) s
     constexpr bool kEven = kTT || kTE || kEE;
     constexpr bool kA2 = kTE || kEE;
     constexpr bool kPk = MASK != M_TT;   // windows and u3 come as pairs (wA, wB)
-    using L = Lay<TS, NW, kPk>;
+    using L = Lay<TS, NW, kPk, DIAG>;
     constexpr int NWL = 2 * (TS - 1) + 32;   // l3 values one stage of a warp covers
     // diagonal tiling: the step factor g[t+j] is the per-lane slice and the column ring g[c-i-t] a broadcast
     constexpr int NG = DIAG ? TS + 31 : TS, NB = DIAG ? TS : TS + 31;
@@ -328,55 +327,21 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB * (128 / SWEEP_THREADS)) s
 #pragma unroll
                     for (int w = 1; w < NW; ++w) xw[w] = pB[w * L::CW].x;
                 }
-                // one block of R steps; TRI: the last block of the walk (diagonal tiling), pairs i < u are finished
-                auto block = [&](auto tri) {
-                    constexpr bool TRI = decltype(tri)::value;
-#pragma unroll
-                    for (int u = 0; u < R; ++u) {
-                        const int i0 = TRI ? u : 0;
-                        wa[(R - u) % R] = xa;
-                        wb[(R + 1 - u) % R] = xb;
-                        const double hg = __dmul_rn(xh, xg);
-                        double q3[NW];
-#pragma unroll
-                        for (int w = 0; w < NW; ++w) q3[w] = __dmul_rn(xw[w], hg);
-                        const double c3 = xu;
-                        xa = pa[-(u + 1)]; xb = pb[-(u + 1)]; xh = ph[-(u + 1)];
-                        // the warp-uniform step factor comes two steps per 16-byte load (the first step is even).  The
-                        // same for the row ring costs more than it saves: its values go into fixed ring registers,
-                        // so half of each pair needs a register move (two instructions) to get there.
-                        if (DIAG) xg = pg[u + 1];   // per lane: plain loads
-                        else if (u % 2 == 0) xg = xg2.y;
-                        else { xg2 = *reinterpret_cast<const double2 *>(pg + (u + 1)); xg = xg2.x; }
-                        {
-                            const double2 v0 = pB[-2 * (u + 1)];
-                            xw[0] = v0.x; xu = v0.y;
-#pragma unroll
-                            for (int w = 1; w < NW; ++w) xw[w] = pB[w * L::CW - 2 * (u + 1)].x;
-                        }
-                        double r[R], e[R];
-#pragma unroll
-                        for (int i = i0; i < R; ++i) r[i] = __dmul_rn(wa[(i - u + R) % R], wb[(2 * R - i - u) % R]);
-                        if (SPIN == 2) {
-#pragma unroll
-                            for (int i = i0; i < R; ++i) e[i] = __dsub_rn(c3, c12[i]);
-#pragma unroll
-                            for (int i = i0; i < R; ++i) r[i] = __dmul_rn(r[i], e[i]);
-#pragma unroll
-                            for (int i = i0; i < R; ++i) r[i] = __dmul_rn(r[i], e[i]);
-                        }
-#pragma unroll
-                        for (int w = 0; w < NW; ++w)
-#pragma unroll
-                            for (int i = i0; i < R; ++i) acc[w][i] = __fma_rn(r[i], q3[w], acc[w][i]);
-                    }
-                    pa -= R; pb -= R; ph -= R; pg += R; pB -= 2 * R;
-                };
+                // blocks of R steps (tj_sweep_odd_block.inc); TRI: the last block of a diagonal-tiling walk
                 const bool tri_last = DIAG && k == nso - 1;
                 const int nfull = tri_last ? nblk - 1 : nblk;
 #pragma unroll 1
-                for (int blk = 0; blk < nfull; ++blk) block(std::false_type{});
-                if constexpr (DIAG) { if (tri_last) block(std::true_type{}); }
+                for (int blk = 0; blk < nfull; ++blk) {
+                    constexpr bool TRI = false;
+#include "tj_sweep_odd_block.inc"
+                    pa -= R; pb -= R; ph -= R; pg += R; pB -= 2 * R;
+                }
+                if constexpr (DIAG) {
+                    if (tri_last) {
+                        constexpr bool TRI = true;
+#include "tj_sweep_odd_block.inc"
+                    }
+                }
                 __syncwarp();
                 if (lane == 0 && q + NBUF < ntot) issue(q + NBUF);
             }
@@ -472,91 +437,21 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB * (128 / SWEEP_THREADS)) s
 #pragma unroll
                 for (int w = 0; w < NW; ++w) { xtt[w] = 0.0; xtp[w] = 0.0; xpp[w] = 0.0; }
                 load_w(0);
-                auto block = [&](auto tri) {   // as in the odd branch
-                    constexpr bool TRI = decltype(tri)::value;
-#pragma unroll
-                    for (int u = 0; u < R; ++u) {
-                        const int i0 = TRI ? u : 0;
-                        wa[(R - u) % R] = xa;
-                        wb[(R + 1 - u) % R] = xb;
-                        const double hg = __dmul_rn(xh, xg);
-                        double q0[NW], q1[NW], q2[NW];
-#pragma unroll
-                        for (int w = 0; w < NW; ++w) {
-                            q0[w] = kTT ? __dmul_rn(xtt[w], hg) : 0.0;
-                            q1[w] = kTE ? __dmul_rn(xtp[w], hg) : 0.0;
-                            q2[w] = kEE ? __dmul_rn(xpp[w], hg) : 0.0;
-                        }
-                        const double c3 = xu;
-                        xa = pa[-(u + 1)]; xb = pb[-(u + 1)]; xh = ph[-(u + 1)];
-                        // the warp-uniform step factor comes two steps per 16-byte load (the first step is even).  The
-                        // same for the row ring costs more than it saves: its values go into fixed ring registers,
-                        // so half of each pair needs a register move (two instructions) to get there.
-                        if (DIAG) xg = pg[u + 1];   // per lane: plain loads
-                        else if (u % 2 == 0) xg = xg2.y;
-                        else { xg2 = *reinterpret_cast<const double2 *>(pg + (u + 1)); xg = xg2.x; }
-                        load_w(-2 * (u + 1));
-                        if (PIPE) {
-                        // accumulate the PREVIOUS step's products first (their inputs are long ready, so the
-                        // 8 FMAs of one window issue back to back and share q through the operand reuse cache)
-#pragma unroll
-                        for (int w = 0; w < NW; ++w) {
-                            if (kTE) {
-#pragma unroll
-                                for (int i = 0; i < R; ++i) ate[w][i] = __fma_rn(rA[i], p1[w], ate[w][i]);
-                            }
-                            if (kEE) {
-#pragma unroll
-                                for (int i = 0; i < R; ++i) aee[w][i] = __fma_rn(rAA[i], p2[w], aee[w][i]);
-                            }
-                            p1[w] = q1[w]; p2[w] = q2[w];
-                        }
-                        }
-                        double r[R], A2[kA2 ? R : 1];
-#pragma unroll
-                        for (int i = i0; i < R; ++i) r[i] = __dmul_rn(wa[(i - u + R) % R], wb[(2 * R - i - u) % R]);
-                        if (kTT) {
-#pragma unroll
-                            for (int w = 0; w < NW; ++w)
-#pragma unroll
-                                for (int i = i0; i < R; ++i) att[w][i] = __fma_rn(r[i], q0[w], att[w][i]);
-                        }
-                        if (kA2) {
-#pragma unroll
-                            for (int i = i0; i < R; ++i) A2[i] = __dsub_rn(c3, c12[i]);
-                            if (SPIN == 2) {
-#pragma unroll
-                                for (int i = i0; i < R; ++i) A2[i] = __fma_rn(A2[i], A2[i], -kk[i]);
-                            }
-#pragma unroll
-                            for (int i = i0; i < R; ++i) rA[i] = __dmul_rn(r[i], A2[i]);
-                            if (kEE) {
-#pragma unroll
-                                for (int i = i0; i < R; ++i) rAA[i] = __dmul_rn(rA[i], A2[i]);
-                            }
-                        }
-                        if (!PIPE) {
-#pragma unroll
-                        for (int w = 0; w < NW; ++w) {
-                            if (kTE) {
-#pragma unroll
-                                for (int i = i0; i < R; ++i) ate[w][i] = __fma_rn(rA[i], q1[w], ate[w][i]);
-                            }
-                            if (kEE) {
-#pragma unroll
-                                for (int i = i0; i < R; ++i) aee[w][i] = __fma_rn(rAA[i], q2[w], aee[w][i]);
-                            }
-                        }
-                        }
-                    }
-                    pa -= R; pb -= R; ph -= R; pg += R;
-                    pwtt -= 2 * R; pA -= 2 * R; pB -= 2 * R;
-                };
                 const bool tri_last = DIAG && k == nse - 1;
                 const int nfull = tri_last ? nblk - 1 : nblk;
 #pragma unroll 1
-                for (int blk = 0; blk < nfull; ++blk) block(std::false_type{});
-                if constexpr (DIAG) { if (tri_last) block(std::true_type{}); }
+                for (int blk = 0; blk < nfull; ++blk) {
+                    constexpr bool TRI = false;
+#include "tj_sweep_even_block.inc"
+                    pa -= R; pb -= R; ph -= R; pg += R;
+                    pwtt -= 2 * R; pA -= 2 * R; pB -= 2 * R;
+                }
+                if constexpr (DIAG) {
+                    if (tri_last) {   // the last block of the walk: pairs i < u are finished
+                        constexpr bool TRI = true;
+#include "tj_sweep_even_block.inc"
+                    }
+                }
                 __syncwarp();
                 if (lane == 0 && q + NBUF < ntot) issue(q + NBUF);
             }
@@ -605,7 +500,7 @@ cudaError_t launch_one(const SweepParams &P, int total_tiles, cudaStream_t st)
     g_last_sweep = SweepGeometry{R, MASK, TS, MINB, PIPE ? 1 : 0, NW, SPIN, ROWS ? 1 : 0, DIAG ? 1 : 0, total_tiles};
     if (total_tiles <= 0) return cudaSuccess;
     constexpr int NWARP = SWEEP_THREADS / 32;
-    constexpr size_t smem = (size_t)NWARP * NBUF * Lay<TS, NW, MASK != M_TT>::BUFD * 8 + (size_t)NWARP * NBUF * 8;
+    constexpr size_t smem = (size_t)NWARP * NBUF * Lay<TS, NW, MASK != M_TT, DIAG>::BUFD * 8 + (size_t)NWARP * NBUF * 8;
     if (smem > 48 * 1024) {   // opt-in beyond the default limit (per device, so not cached; one-warp CTAs stay below it)
         cudaError_t e = cudaFuncSetAttribute(sweep_tma_kernel<R, MASK, TS, MINB, PIPE, NW, SPIN, ROWS, DIAG>,
                                              cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);

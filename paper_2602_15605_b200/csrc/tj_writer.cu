@@ -123,23 +123,28 @@ cudaError_t launch_scale_rows(double *const M[4], int nmat, double *bb, int bb_s
     return cudaGetLastError();
 }
 
-// One CTA: rows r0..r0+31 of ONE banded output, deltas d0..d0+31.
-//   direct:  M[r][lcut+delta] = (2(r+delta)+1) Xi(r, r+delta)          source X[delta][r]
-//   mirror:  M[r][lcut-delta] = (2(r-delta)+1) Xi(r-delta, r)          source X[delta][r-delta]   (delta >= 1)
-// Both sources are read as 32 consecutive doubles per delta and transposed through shared memory.
-__global__ void __launch_bounds__(WT * WROWS) band_writer_kernel(const __grid_constant__ BandWriterParams P)
+// One CTA: deltas d0..d0+31 of ONE banded output, and
+//   direct:  rows l1 = r0..r0+31:       M[l1][lcut+delta] = (2(l1+delta)+1) Xi(l1, l1+delta)   source X[delta][l1]
+//   mirror:  rows r = r0+d0..r0+d0+31:  M[r][lcut-delta]  = (2(r-delta)+1)  Xi(r-delta, r)     source X[delta][r-delta]
+// Both are 32 consecutive columns per row, and both sources are read as 32 consecutive doubles per delta and
+// transposed through shared memory.  The mirror rows are shifted by d0 against the direct rows so that the two source
+// tiles cover the same l1 range (r0-31..r0+31): the second read of an element comes from L2, not from HBM.
+// (delta = 0: one slot, written by the direct part.)  Slots whose l2 falls outside 0..lmax get 0.0; CTAs of negative
+// r0 (blockIdx.y below y0) only write the mirror-side zeros of the rows r < delta.  Every slot is written exactly once.
+__global__ void __launch_bounds__(WT * WROWS) band_writer_kernel(const __grid_constant__ BandWriterParams P, int y0)
 {
     __shared__ double td[WT][WT + 1], tm[WT][WT + 1];
     const int tx = threadIdx.x, ty = threadIdx.y;
-    const int d0 = blockIdx.x * WT, r0 = blockIdx.y * WT, m = blockIdx.z;
+    const int d0 = blockIdx.x * WT, r0 = ((int)blockIdx.y - y0) * WT, m = blockIdx.z;
+    if (r0 < 0 && r0 + d0 + WT - 1 < 0) return;   // neither direct rows nor mirror rows
     const double *X = P.X[m];
     double *M = P.M[m];
     double *bb = (P.bb != nullptr && m == P.bb_src) ? P.bb : nullptr;
 #pragma unroll
     for (int k = ty; k < WT; k += WROWS) {
         const int delta = d0 + k;
-        const int l1d = r0 + tx, l1m = r0 - delta + tx;
-        const bool okd = delta <= P.dmax && l1d + delta <= P.lmax;
+        const int l1d = r0 + tx, l1m = r0 - k + tx;
+        const bool okd = delta <= P.dmax && l1d >= 0 && l1d + delta <= P.lmax;
         const bool okm = delta <= P.dmax && delta >= 1 && l1m >= 0 && l1m + delta <= P.lmax;
         td[k][tx] = okd ? X[(long long)delta * P.ldT + l1d] : 0.0;
         tm[k][tx] = okm ? X[(long long)delta * P.ldT + l1m] : 0.0;
@@ -149,19 +154,20 @@ __global__ void __launch_bounds__(WT * WROWS) band_writer_kernel(const __grid_co
     if (delta > P.lcut) return;
 #pragma unroll
     for (int k = ty; k < WT; k += WROWS) {
-        const int r = r0 + k;
-        if (r > P.lmax) break;
-        const long long row = (long long)r * P.ld + P.lcut;
-        {   // out-of-range slots read 0.0 from the tile: 0.0 * (2 l2+1) = 0.0
-            const double v = td[tx][k] * (double)(2 * (r + delta) + 1);
-            M[row + delta] = v;
-            if (bb) bb[row + delta] = v;
+        const int l1 = r0 + k;           // direct row
+        if (l1 >= 0 && l1 <= P.lmax) {
+            const double v = td[tx][k] * (double)(2 * (l1 + delta) + 1);   // out of range: 0.0 * positive = 0.0
+            const long long ix = (long long)l1 * P.ld + P.lcut + delta;
+            M[ix] = v;
+            if (bb) bb[ix] = v;
         }
-        if (delta >= 1) {
-            const double v = tm[tx][k] * (double)(2 * (r - delta) + 1);
-            const double w = (r - delta >= 0) ? v : 0.0;   // (a negative factor times 0.0 would store -0.0)
-            M[row - delta] = w;
-            if (bb) bb[row - delta] = w;
+        const int r = r0 + d0 + k;       // mirror row; its source row of Xi is l1 = r - delta = r0 + k - tx
+        if (delta >= 1 && r >= 0 && r <= P.lmax) {
+            const int lm = r - delta;
+            const double v = lm >= 0 ? tm[tx][k] * (double)(2 * lm + 1) : 0.0;
+            const long long ix = (long long)r * P.ld + P.lcut - delta;
+            M[ix] = v;
+            if (bb) bb[ix] = v;
         }
     }
 }
@@ -169,8 +175,9 @@ __global__ void __launch_bounds__(WT * WROWS) band_writer_kernel(const __grid_co
 cudaError_t launch_band_writer(const BandWriterParams &P, cudaStream_t st)
 {
     if (P.nmat <= 0) return cudaSuccess;
-    dim3 grid((unsigned)(P.lcut / WT + 1), (unsigned)((P.lmax + WT) / WT), (unsigned)P.nmat);
-    band_writer_kernel<<<grid, dim3(WT, WROWS, 1), 0, st>>>(P);
+    const int y0 = (P.lcut + WT - 1) / WT;   // tiles of negative l1: the zeros of the rows r < delta
+    dim3 grid((unsigned)(P.lcut / WT + 1), (unsigned)(y0 + (P.lmax + WT) / WT), (unsigned)P.nmat);
+    band_writer_kernel<<<grid, dim3(WT, WROWS, 1), 0, st>>>(P, y0);
     ++g_launch_count;
     return cudaGetLastError();
 }
