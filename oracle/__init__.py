@@ -19,6 +19,7 @@ from .coupling import (  # noqa: F401
     coupling_rows,
     coupling_full,
     coupling_band,
+    coupling_binned,
     spin1_pairs,
     spin1_full,
     num_threads,

@@ -187,3 +187,38 @@ def spin1_full(lmax, l3max, W01, W11):
     l1s = np.repeat(np.arange(N, dtype=np.int32), N)
     l2s = np.tile(np.arange(N, dtype=np.int32), N)
     return {k: v.reshape(N, N) for k, v in spin1_pairs(l3max, W01, W11, l1s, l2s).items()}
+
+
+def coupling_binned(lmax, l3max, Wtt, Wtp, Wpp, edges, P, Q, pairs=None):
+    """Binned matrices (reading 20; the paper prints no binning operator):
+
+        B^{XY}[b][b'] = sum_{l1 in bin b} sum_{l2 in bin b'} P[l1] K^{XY}[l1][l2] Q[l2],
+
+    bin b = edges[b] <= l < edges[b+1] (ascending, within 0..lmax+1), P and Q per-l weights with lmax+1 entries:
+    the sum of the oracle's own entries, written out (every entry from its definition, no symmetry).
+    `pairs`: list of (b, b') to evaluate (default: all); the others are returned as NaN.
+    Returns dict name -> float64[nbins, nbins]."""
+    edges = np.asarray(edges, dtype=np.int64)
+    nb = edges.size - 1
+    assert nb >= 1 and edges[0] >= 0 and edges[-1] <= lmax + 1 and np.all(np.diff(edges) >= 0)
+    P = np.ascontiguousarray(P, dtype=np.float64)
+    Q = np.ascontiguousarray(Q, dtype=np.float64)
+    assert P.shape == (lmax + 1,) and Q.shape == (lmax + 1,)
+    if pairs is None:
+        pairs = [(b, c) for b in range(nb) for c in range(nb)]
+    names = [k for k, w in (("TT", Wtt), ("TE", Wtp), ("EE", Wpp), ("BB", Wpp), ("EB", Wpp)) if w is not None]
+    out = {k: np.full((nb, nb), np.nan) for k in names}
+    for b, c in pairs:
+        r = np.arange(edges[b], edges[b + 1], dtype=np.int32)
+        q = np.arange(edges[c], edges[c + 1], dtype=np.int32)
+        if r.size == 0 or q.size == 0:
+            for k in names:
+                out[k][b, c] = 0.0
+            continue
+        l1 = np.repeat(r, q.size)
+        l2 = np.tile(q, r.size)
+        K = coupling_pairs(l3max, Wtt, Wtp, Wpp, l1, l2)
+        wgt = (P[r][:, None] * Q[q][None, :]).ravel()
+        for k in names:
+            out[k][b, c] = float(np.sum(wgt * K[k]))
+    return out
