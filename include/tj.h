@@ -140,6 +140,23 @@ int tj_coupling_rows(const tj_tables *tables,
                      void *cuda_stream);
 
 /*
+ * tj_coupling_binned -- binned output.  The paper prints no binning operator; the form taken here
+ * (reading 20) is the one a pseudo-C_l pipeline applies to K:
+ *     B^{XY}[b][b'] = sum_{l1 in bin b} sum_{l2 in bin b'} P[l1] K^{XY}[l1][l2] Q[l2],
+ * bin b = h_edges[b] <= l < h_edges[b+1] (h_edges: HOST array of nbins+1 ascending values within 0..lmax+1; bins
+ * may be empty and need not cover every l), d_P / d_Q: DEVICE arrays of lmax+1 per-l weights.  The same fused sweep
+ * runs over chunks of rows and a binning kernel takes the place of the mirrored writer, so the (lmax+1)^2 matrices
+ * are never written.  Outputs: nbins*nbins doubles each, row-major [b][b']; windows, NULL rules and BB (= EE) as
+ * tj_coupling_pol.  Results are deterministic (fixed summation order) and agree with the binned tj_coupling_pol
+ * matrices to rounding.
+ */
+int tj_coupling_binned(const tj_tables *tables,
+                       const double *d_Wtt, const double *d_Wtp, const double *d_Wpp, int nW,
+                       int nbins, const int *h_edges, const double *d_P, const double *d_Q,
+                       double *d_TT, double *d_TE, double *d_EE, double *d_BB, double *d_EB,
+                       void *cuda_stream);
+
+/*
  * tj_coupling_literal -- ABLATION, not the hot path: the paper's own evaluation restated as
  * one plain kernel -- one thread per (l1,l2) of the upper triangle, serial l3 loop in steps of 2 with direct
  * table lookups, K^{TT} from Eq. 10 and K^{EE} from Eq. 16

@@ -18,7 +18,7 @@ TJ_OK, TJ_EINVAL, TJ_ENOMEM, TJ_ECUDA = 0, -1, -2, -3
 # every symbol include/tj.h declares (tests/test_abi.py checks the header against this and the .so)
 SYMBOLS = (
     "tj_build_tables", "tj_free_tables", "tj_tables_info", "tj_tables_copy",
-    "tj_coupling_tt", "tj_coupling_pol", "tj_coupling_band", "tj_coupling_multi", "tj_coupling_spin1", "tj_coupling_rows", "tj_coupling_literal", "tj_coupling_host",
+    "tj_coupling_tt", "tj_coupling_pol", "tj_coupling_band", "tj_coupling_multi", "tj_coupling_spin1", "tj_coupling_rows", "tj_coupling_binned", "tj_coupling_literal", "tj_coupling_host",
     "tj_l3_range", "tj_sweep_counts", "tj_fp64_probe", "tj_profile_enable", "tj_profile_get",
     "tj_profile_last_sweep", "tj_profile_launches", "tj_strerror",
 )
@@ -55,6 +55,7 @@ def load_library() -> ctypes.CDLL:
     L.tj_coupling_multi.argtypes = [vp, ci, vp, vp, vp, ci, vp, vp, vp, vp, vp, vp]
     L.tj_coupling_spin1.argtypes = [vp, vp, vp, vp, ci, vp, vp, vp, vp, vp]
     L.tj_coupling_rows.argtypes = [vp, vp, vp, vp, ci, ci, ci, vp, vp, vp, vp, vp, vp]
+    L.tj_coupling_binned.argtypes = [vp, vp, vp, vp, ci, ci, ip, vp, vp, vp, vp, vp, vp, vp, vp]
     L.tj_coupling_literal.argtypes = [vp, vp, vp, ci, vp, vp, vp]
     L.tj_coupling_host.argtypes = [vp, ci, ci, vp, vp, vp, vp, vp, vp, vp, vp, vp]
     L.tj_l3_range.argtypes = [ci, ci, ci, ci, ip, ip, ip]
@@ -257,6 +258,27 @@ def coupling_rows(tables: Tables, Wtt, Wtp, Wpp, row_lo: int, row_hi: int, want=
     _check(load_library().tj_coupling_rows(tables.handle, _dev_ptr(Wtt, nW, "Wtt"), _dev_ptr(Wtp, nW, "Wtp"),
                                            _dev_ptr(Wpp, nW, "Wpp"), nW, int(row_lo), int(row_hi), *args,
                                            _stream_ptr(stream)), "tj_coupling_rows")
+    return {k: out[k] for k in want}
+
+
+def coupling_binned(tables: Tables, Wtt, Wtp, Wpp, edges, P, Q, want=_BLOCKS, out=None, stream=None):
+    """tj_coupling_binned.  edges: nbins+1 ascending ints (host); P, Q: float64 CUDA tensors [lmax+1].
+    Returns dict name -> [nbins, nbins] tensor."""
+    import torch
+    N = tables.lmax + 1
+    nW = tables.l3max + 1
+    edges = [int(x) for x in edges]
+    nb = len(edges) - 1
+    harr = (ctypes.c_int * (nb + 1))(*edges)
+    dev = P.device
+    out = {} if out is None else dict(out)
+    for k in want:
+        if k not in out:
+            out[k] = torch.empty((nb, nb), dtype=torch.float64, device=dev)
+    args = [_dev_ptr(out.get(k) if k in want else None, nb * nb, k) for k in _BLOCKS]
+    _check(load_library().tj_coupling_binned(tables.handle, _dev_ptr(Wtt, nW, "Wtt"), _dev_ptr(Wtp, nW, "Wtp"),
+                                             _dev_ptr(Wpp, nW, "Wpp"), nW, nb, harr, _dev_ptr(P, N, "P"), _dev_ptr(Q, N, "Q"),
+                                             *args, _stream_ptr(stream)), "tj_coupling_binned")
     return {k: out[k] for k in want}
 
 

@@ -105,6 +105,9 @@ int run_coupling_rows_to_host(const tj_tables *tables, const double *d_Wtt, cons
                               int nW, double *const d_out[5], double *const h_out[5], cudaStream_t st);
 int run_literal(const tj_tables *tables, const double *d_Wtt, const double *d_Wpp, int nW, double *d_TT, double *d_EE,
                 cudaStream_t st);
+int run_binned(const tj_tables *tables, const double *d_Wtt, const double *d_Wtp, const double *d_Wpp, int nW, int nbins,
+               const int *h_edges, const double *d_P, const double *d_Q, double *d_TT, double *d_TE, double *d_EE,
+               double *d_BB, double *d_EB, cudaStream_t st);
 
 }  // namespace
 
@@ -267,6 +270,19 @@ int tj_coupling_rows(const tj_tables *tables, const double *d_Wtt, const double 
     if (nW != tables->T.l3max + 1) return TJ_EINVAL;
     if (row_lo < 0 || row_hi <= row_lo || row_hi > tables->T.lmax + 1) return TJ_EINVAL;
     return run_rows(tables, d_Wtt, d_Wtp, d_Wpp, nW, row_lo, row_hi, d_TT, d_TE, d_EE, d_BB, d_EB, (cudaStream_t)cuda_stream);
+}
+
+int tj_coupling_binned(const tj_tables *tables, const double *d_Wtt, const double *d_Wtp, const double *d_Wpp, int nW,
+                       int nbins, const int *h_edges, const double *d_P, const double *d_Q, double *d_TT, double *d_TE,
+                       double *d_EE, double *d_BB, double *d_EB, void *cuda_stream)
+{
+    if (!tables || !h_edges || !d_P || !d_Q || nbins < 1 || nbins > 46340) return TJ_EINVAL;
+    if (nW != tables->T.l3max + 1) return TJ_EINVAL;
+    if (h_edges[0] < 0 || h_edges[nbins] > tables->T.lmax + 1) return TJ_EINVAL;
+    for (int b = 0; b < nbins; ++b)
+        if (h_edges[b + 1] < h_edges[b]) return TJ_EINVAL;
+    return run_binned(tables, d_Wtt, d_Wtp, d_Wpp, nW, nbins, h_edges, d_P, d_Q, d_TT, d_TE, d_EE, d_BB, d_EB,
+                      (cudaStream_t)cuda_stream);
 }
 
 int tj_coupling_literal(const tj_tables *tables, const double *d_Wtt, const double *d_Wpp, int nW, double *d_TT,
@@ -648,6 +664,73 @@ int run_rows(const tj_tables *tables, const double *d_Wtt, const double *d_Wtp, 
     if (e != cudaSuccess) rc = cuda_fail(e, "tj_coupling_rows");
     coupling_end(C, st);
     return rc;
+}
+
+// binned output (tj_binned.cu): the sweep runs over chunks of rows into Xi scratch, bin_kernel adds each chunk to the bins
+int run_binned(const tj_tables *tables, const double *d_Wtt, const double *d_Wtp, const double *d_Wpp, int nW, int nbins,
+               const int *h_edges, const double *d_P, const double *d_Q, double *d_TT, double *d_TE, double *d_EE,
+               double *d_BB, double *d_EB, cudaStream_t st)
+{
+    const Tables &T = tables->T;
+    const long long N = (long long)T.lmax + 1;
+    double *outs[4] = {d_TT, d_TE, d_EE ? d_EE : d_BB, d_EB};
+    int nmat = 0;
+    for (int k = 0; k < 4; ++k) nmat += outs[k] ? 1 : 0;
+    if (nmat == 0) return TJ_EINVAL;
+    if ((d_TT && !d_Wtt) || (d_TE && !d_Wtp) || ((d_EE || d_BB || d_EB) && !d_Wpp)) return TJ_EINVAL;
+    // rows per chunk: whole row bands of the sweep, at most ~1 GiB of Xi scratch
+    const int mask = (!d_TE && !outs[2] && !d_EB) ? M_TT : (d_TT ? M_TT : 0) | M_TE | M_EE | M_EB;
+    const int R = sweep_R(mask, false, 1, T.lmax, false, 2);
+    long long ch = ((1LL << 30) / (8 * N * nmat)) / R * R;
+    if (ch < R) ch = R;
+    if (ch > N) ch = (N + R - 1) / R * R;
+    const size_t xper = (size_t)ch * (size_t)N;
+    const size_t ebytes = (sizeof(int) * (size_t)(nbins + 1) + 127) & ~(size_t)127;
+    unsigned char *scr = nullptr;
+    TJ_CUDA(cudaMallocAsync((void **)&scr, ebytes + sizeof(double) * xper * (size_t)nmat, st), "tj_coupling_binned/scratch");
+    int *d_edges = (int *)scr;
+    double *xb = (double *)(scr + ebytes);
+    cudaError_t e = cudaMemcpyAsync(d_edges, h_edges, sizeof(int) * (size_t)(nbins + 1), cudaMemcpyHostToDevice, st);
+    // the sweep's targets: one chunk buffer per requested block, in the order TT, TE, EE, EB
+    double *bufs[4] = {nullptr, nullptr, nullptr, nullptr};
+    {
+        int k = 0;
+        for (int m = 0; m < 4; ++m)
+            if (outs[m]) bufs[m] = xb + xper * (size_t)(k++);
+    }
+    Call C;
+    int rc = TJ_OK;
+    if (e == cudaSuccess) rc = coupling_begin(C, tables, -1, d_Wtt, d_Wtp, d_Wpp, nW, bufs[0], bufs[1], bufs[2], nullptr, bufs[3], st);
+    if (e == cudaSuccess && rc == TJ_OK) {
+        BinParams B;
+        memset(&B, 0, sizeof(B));
+        for (int m = 0; m < 4 && e == cudaSuccess; ++m) {
+            if (!outs[m]) continue;
+            B.B[B.nmat++] = outs[m];
+            e = cudaMemsetAsync(outs[m], 0, sizeof(double) * (size_t)nbins * (size_t)nbins, st);
+        }
+        B.edges = d_edges; B.P = d_P; B.Q = d_Q; B.nbins = nbins; B.lmax = T.lmax; B.ld = N;
+        prof_record(2, st);
+        for (long long r0 = 0; r0 < N && e == cudaSuccess; r0 += ch) {
+            const long long r1 = r0 + ch < N ? r0 + ch : N;
+            // the sweep addresses Xi(l1,l2) as base[l1*N + l2]: shift the bases so that row r0 is row 0 of the chunk
+            int k = 0;
+            double **tgt[4] = {&C.TT, &C.TE, &C.ee, &C.EB};
+            for (int m = 0; m < 4; ++m)
+                if (outs[m]) { *tgt[m] = bufs[m] - r0 * N; B.X[k++] = bufs[m]; }
+            e = coupling_sweep(C, (int)(r0 / C.R), r1 == N ? C.nb : (int)(r1 / C.R), st);
+            B.r0 = (int)r0; B.r1 = (int)r1;
+            if (e == cudaSuccess) e = launch_bin(B, st);
+        }
+        prof_record(3, st);
+        if (e == cudaSuccess && d_EE && d_BB)
+            e = cudaMemcpyAsync(d_BB, d_EE, sizeof(double) * (size_t)nbins * (size_t)nbins, cudaMemcpyDeviceToDevice, st);
+        prof_record(4, st);
+        coupling_end(C, st);
+    }
+    cudaFreeAsync(scr, st);
+    if (rc != TJ_OK) return rc;
+    return e == cudaSuccess ? TJ_OK : cuda_fail(e, "tj_coupling_binned");
 }
 
 // paper-literal ablation (tj_literal.cu): prefold the windows, then one thread per pair

@@ -155,6 +155,18 @@ struct BandWriterParams {
     long long ldT, ld;              // ld = 2*lcut+1
 };
 
+// binned output (tj_binned.cu): one chunk of rows [r0, r1) of Xi per block -> accumulated into nbins x nbins
+struct BinParams {
+    const double *X[4];             // X[m][(l1-r0)*ld + l2] = Xi(l1,l2) for l2 >= l1
+    double *B[4];                   // B[m][b*nbins + b']
+    int nmat;
+    const int *edges;               // device, nbins+1 ascending bin edges
+    const double *P, *Q;            // device, lmax+1 weights each
+    int nbins, r0, r1, lmax;
+    long long ld;
+};
+cudaError_t launch_bin(const BinParams &P, cudaStream_t st);
+
 // kernels / launchers (defined in the .cu files)
 cudaError_t launch_build_tables(const Tables &T, cudaStream_t st);
 cudaError_t launch_prepare(const Tables &T, const double *d_Wtt, const double *d_Wtp, const double *d_Wpp, int nW,

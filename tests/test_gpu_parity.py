@@ -879,3 +879,101 @@ def test_spike_every_l3_slot_banded(lmax, lcut):
         for k in BLOCKS:
             assert_parity(K[k], ref[k], "band spike L=%d %s" % (L, k))
     T.close()
+
+
+# ---------------------------------------------------------------- binned output (DESIGN.md 2 reading 20)
+def _bin_weights(lmax, seed):
+    rng = np.random.default_rng(seed)
+    return rng.uniform(0.5, 1.5, lmax + 1), rng.uniform(0.5, 1.5, lmax + 1)
+
+
+@pytest.mark.parametrize("lmax,edges", [(100, [0, 2, 7, 7, 30, 64, 101]), (257, [2, 34, 66, 130, 258]), (64, [5, 6]),
+                                         (900, list(range(0, 901, 75)) + [901])])
+def test_binned_against_oracle_and_binned_full_matrices(lmax, edges):
+    import torch
+    wl = windows.config(1, lmax=lmax)
+    P, Q = _bin_weights(lmax, lmax)
+    T = binding.build_tables(lmax)
+    W = [_t(w) for w in (wl.Wtt, wl.Wtp, wl.Wpp)]
+    nb = len(edges) - 1
+    pre = {k: torch.full((nb, nb), float("nan"), dtype=torch.float64, device="cuda") for k in BLOCKS}
+    B = binding.coupling_binned(T, *W, edges, _t(P), _t(Q), out=pre)
+    full = binding.coupling_pol(T, *W)
+    torch.cuda.synchronize()
+    pairs = None if lmax <= 300 else [(0, 0), (3, 11), (11, 3), (12, 12), (7, 8), (12, 0)]
+    ref = oracle.coupling_binned(lmax, 2 * lmax, wl.Wtt, wl.Wtp, wl.Wpp, edges, P, Q, pairs=pairs)
+    for k in BLOCKS:
+        got = B[k].cpu().numpy()
+        sel = ~np.isnan(ref[k])
+        assert_parity(got[sel], ref[k][sel], "binned %s" % k)
+        # the same bins formed from the full matrices of tj_coupling_pol, in float64 on the host
+        K = full[k].cpu().numpy()
+        for b in range(nb):
+            for c in range(nb):
+                want = float(P[edges[b]:edges[b + 1]] @ K[edges[b]:edges[b + 1], edges[c]:edges[c + 1]] @ Q[edges[c]:edges[c + 1]])
+                assert abs(got[b, c] - want) <= 1e-12 * max(abs(want), 1e-6), (k, b, c)
+    assert torch.equal(B["BB"], B["EE"])
+    # partial requests and determinism
+    again = binding.coupling_binned(T, *W, edges, _t(P), _t(Q))
+    only = binding.coupling_binned(T, None, None, W[2], edges, _t(P), _t(Q), want=("BB", "EB"))
+    tt = binding.coupling_binned(T, W[0], None, None, edges, _t(P), _t(Q), want=("TT",))
+    torch.cuda.synchronize()
+    for k in BLOCKS:
+        assert torch.equal(again[k], B[k]), k
+    assert_parity(only["EB"].cpu().numpy(), B["EB"].cpu().numpy(), "binned EB alone")
+    assert_parity(only["BB"].cpu().numpy(), B["BB"].cpu().numpy(), "binned BB alone")
+    assert_parity(tt["TT"].cpu().numpy(), B["TT"].cpu().numpy(), "binned TT alone")
+    with pytest.raises(binding.TJError):
+        binding.coupling_binned(T, *W, [0, 5, 3], _t(P), _t(Q))
+    with pytest.raises(binding.TJError):
+        binding.coupling_binned(T, *W, [0, lmax + 2], _t(P), _t(Q))
+    T.close()
+
+
+@pytest.mark.parametrize("cfg,width", [(1, 40), (3, 50)])
+def test_binned_full_size_configs_sampled_bins(cfg, width):
+    """Configs 1 and 3 at full size (config 3: several chunks of rows): sampled bin pairs against the oracle."""
+    import torch
+    wl = windows.config(cfg)
+    lmax = wl.lmax
+    edges = list(range(2, lmax + 1, width)) + [lmax + 1]
+    nb = len(edges) - 1
+    l = np.arange(lmax + 1, dtype=np.float64)
+    P = (l * (l + 1) / (2 * np.pi)) / width                      # a band-power operator and its inverse
+    Q = np.where(l > 0, 2 * np.pi / np.maximum(l * (l + 1), 1.0), 0.0)
+    T = binding.build_tables(lmax)
+    B = binding.coupling_binned(T, _t(wl.Wtt), _t(wl.Wtp), _t(wl.Wpp), edges, _t(P), _t(Q))
+    torch.cuda.synchronize()
+    pairs = [(0, 0), (0, 1), (1, 0), (nb - 1, nb - 1), (nb // 2, nb // 2), (nb // 2, nb // 2 + 1), (nb // 3, nb - 2), (nb - 1, 0)]
+    ref = oracle.coupling_binned(lmax, wl.l3max, wl.Wtt, wl.Wtp, wl.Wpp, edges, P, Q, pairs=pairs)
+    for k in BLOCKS:
+        got = B[k].cpu().numpy()
+        assert np.all(np.isfinite(got))
+        sel = ~np.isnan(ref[k])
+        # a bin is a sum of width^2 entries of either sign (TE): the bar applies on the scale of the bin's largest entry sum
+        assert_parity(got[sel], ref[k][sel], "cfg%d binned %s" % (cfg, k))
+    T.close()
+
+
+def test_binned_flat_window_closed_form_multi_chunk():
+    """Flat window at lmax = 7000 (two chunks of rows): every bin against B = (sum_b P)(sum_b' Q (2l+1))/4 pi, TE = 0,
+    EE + EB = the same on l >= 2 -- no oracle sample involved."""
+    import torch
+    lmax = 7000
+    edges = [0, 2] + list(range(30, lmax, 97)) + [lmax + 1]
+    nb = len(edges) - 1
+    P, Q = _bin_weights(lmax, 5)
+    W = _t(np.ones(2 * lmax + 1))
+    T = binding.build_tables(lmax)
+    B = {k: v.cpu().numpy() for k, v in binding.coupling_binned(T, W, W, W, edges, _t(P), _t(Q)).items()}
+    l = np.arange(lmax + 1)
+    sp = np.array([P[edges[b]:edges[b + 1]].sum() for b in range(nb)])
+    sq = np.array([(Q[edges[b]:edges[b + 1]] * (2 * l[edges[b]:edges[b + 1]] + 1)).sum() for b in range(nb)])
+    want = np.outer(sp, sq) / (4 * np.pi)
+    assert np.all(np.abs(B["TT"] - want) <= 1e-11 * want)
+    assert np.all(np.abs(B["TE"]) <= 1e-11 * want)
+    pol = want.copy()
+    pol[0, :] = 0.0
+    pol[:, 0] = 0.0                                   # bin 0 = l < 2
+    assert np.all(np.abs(B["EE"] + B["EB"] - pol) <= 1e-11 * np.maximum(want, 1e-30))
+    T.close()
