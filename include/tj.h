@@ -33,8 +33,12 @@ extern "C" {
 #define TJ_ENOMEM  (-2)  /* host or device allocation failed */
 #define TJ_ECUDA   (-3)  /* CUDA runtime / launch error; text via tj_strerror(TJ_ECUDA) */
 
-/* Opaque handle owning the device-resident lookup tables for one (lmax, l3max).  Immutable after
- * build, so it may be used concurrently from several streams. */
+/* Opaque handle owning the device-resident lookup tables for one (lmax, l3max) on ONE device: the device that is
+ * current when tj_build_tables is called.  Every later call with the handle must be made with the same device
+ * current (TJ_EINVAL otherwise); one process can drive several GPUs with one handle per device.  The tables are
+ * immutable after build, so a handle may be used concurrently from several streams and threads (host-buffer
+ * calls that share a handle are serialised inside the library).  tj_free_tables also releases the side streams
+ * the host-buffer calls created for the handle. */
 typedef struct tj_tables tj_tables;
 
 /*
@@ -201,7 +205,7 @@ int tj_sweep_counts(int l1, int l2, int l3max, int *te_lo, int *te_hi, int *to_l
 
 /*
  * tj_fp64_probe -- measurement aid for the roofline denominator: runs `iters` dependent-chain DFMA
- * iterations of 8 independent chains per thread on every SM and returns, through *h_thread_instr_per_s,
+ * iterations of 16 independent chains per thread on every SM and returns, through *h_thread_instr_per_s,
  * the achieved FP64 thread-instructions per second (synchronous; CUDA-event timed).
  */
 int tj_fp64_probe(int iters, void *cuda_stream, double *h_thread_instr_per_s);

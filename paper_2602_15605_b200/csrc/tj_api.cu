@@ -28,19 +28,49 @@ int cuda_fail(cudaError_t e, const char *where)
         if (e__ != cudaSuccess) return cuda_fail(e__, where);  \
     } while (0)
 
-// keep freed scratch in the default mem pool instead of returning it to the OS after every call
-void tune_pool_once()
+// keep freed scratch in the device's default mem pool instead of returning it to the OS after every call
+// (per device: called from every tj_build_tables; setting the attribute again is harmless)
+void tune_pool(int dev)
 {
-    static std::once_flag once;
-    std::call_once(once, [] {
-        int dev = 0;
-        if (cudaGetDevice(&dev) != cudaSuccess) return;
-        cudaMemPool_t pool;
-        if (cudaDeviceGetDefaultMemPool(&pool, dev) != cudaSuccess) return;
-        unsigned long long thr = ~0ull;
-        cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &thr);
-    });
+    cudaMemPool_t pool;
+    if (cudaDeviceGetDefaultMemPool(&pool, dev) != cudaSuccess) return;
+    unsigned long long thr = ~0ull;
+    cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &thr);
 }
+
+// Side streams and events of the host-buffer pipeline (run_coupling_rows_to_host).  They belong to a tables handle,
+// i.e. to ONE device: created on first use, destroyed by tj_free_tables; the mutex serialises host-buffer calls that
+// share a handle (each of them synchronises before it returns anyway).
+constexpr int PIPE_MAX_CHUNKS = 24;
+struct HostPipe {
+    std::mutex mu;
+    cudaStream_t comp[2] = {nullptr, nullptr}, copy = nullptr;
+    cudaEvent_t ev[PIPE_MAX_CHUNKS + 2];
+    int nev = 0;
+    bool have = false;
+    cudaError_t ensure()
+    {
+        if (have) return cudaSuccess;
+        cudaError_t e = cudaSuccess;
+        for (int k = 0; k < 2 && e == cudaSuccess; ++k) e = cudaStreamCreateWithFlags(&comp[k], cudaStreamNonBlocking);
+        if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&copy, cudaStreamNonBlocking);
+        for (int k = 0; k < PIPE_MAX_CHUNKS + 2 && e == cudaSuccess; ++k) {
+            e = cudaEventCreateWithFlags(&ev[k], cudaEventDisableTiming);
+            if (e == cudaSuccess) ++nev;
+        }
+        if (e != cudaSuccess) { destroy(); return e; }
+        have = true;
+        return cudaSuccess;
+    }
+    void destroy()
+    {
+        for (int k = 0; k < nev; ++k) cudaEventDestroy(ev[k]);
+        nev = 0;
+        for (int k = 0; k < 2; ++k) if (comp[k]) { cudaStreamDestroy(comp[k]); comp[k] = nullptr; }
+        if (copy) { cudaStreamDestroy(copy); copy = nullptr; }
+        have = false;
+    }
+};
 
 // optional per-kernel timing of the most recent coupling call of this thread (tj_profile_*)
 std::atomic<int> g_profile{0};
@@ -113,7 +143,20 @@ int run_binned(const tj_tables *tables, const double *d_Wtt, const double *d_Wtp
 
 struct tj_tables {
     Tables T;
+    int device = 0;     // the device the tables live on; every entry point checks that it is the current one
+    HostPipe pipe;
 };
+
+namespace {
+// TJ_EINVAL unless the handle's device is the calling thread's current device (streams, scratch and kernels of a call
+// all belong to the current device: a handle built on another GPU cannot be used without cudaSetDevice)
+int check_device(const tj_tables *tables)
+{
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess) return cuda_fail(cudaGetLastError(), "cudaGetDevice");
+    return dev == tables->device ? TJ_OK : TJ_EINVAL;
+}
+}  // namespace
 
 extern "C" {
 
@@ -156,8 +199,9 @@ int tj_build_tables(int lmax, int l3max, void *cuda_stream, tj_tables **out)
     T.isu = p;
     e = launch_build_tables(T, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e == cudaSuccess) e = cudaGetDevice(&h->device);
     if (e != cudaSuccess) { cudaFree(T.base); delete h; return cuda_fail(e, "tj_build_tables"); }
-    tune_pool_once();
+    tune_pool(h->device);
     *out = h;
     return TJ_OK;
 }
@@ -165,6 +209,7 @@ int tj_build_tables(int lmax, int l3max, void *cuda_stream, tj_tables **out)
 void tj_free_tables(tj_tables *tables)
 {
     if (!tables) return;
+    tables->pipe.destroy();
     cudaFree(tables->T.base);
     delete tables;
 }
@@ -196,6 +241,7 @@ int tj_tables_copy(const tj_tables *tables, int which, double *h_dst, int count)
         default: return TJ_EINVAL;
     }
     if (count > maxn) return TJ_EINVAL;
+    { const int rcd = check_device(tables); if (rcd != TJ_OK) return rcd; }
     TJ_CUDA(cudaMemcpy(h_dst, src, sizeof(double) * (size_t)count, cudaMemcpyDeviceToHost), "tj_tables_copy");
     return TJ_OK;
 }
@@ -315,7 +361,7 @@ int tj_coupling_host(const tj_tables *tables, int band, int nW_or_lcut, const do
     int nout = 0;
     for (int k = 0; k < 5; ++k) if (ho[k] && !(k == 3 && bb_from_ee)) ++nout;
     if (nout == 0) return TJ_EINVAL;
-    tune_pool_once();
+    { const int rcd = check_device(tables); if (rcd != TJ_OK) return rcd; }
     double *dw = nullptr, *dout = nullptr;
     TJ_CUDA(cudaMallocAsync((void **)&dw, sizeof(double) * 3 * (size_t)nW, st), "tj_coupling_host/alloc windows");
     cudaError_t e = cudaMallocAsync((void **)&dout, sizeof(double) * per * (size_t)nout, st);
@@ -463,6 +509,7 @@ int coupling_begin(Call &C, const tj_tables *tables, int lcut, const double *d_W
                    cudaStream_t st, int nw = 1, int spin = 2, int row_lo = -1, int row_hi = -1)
 {
     const Tables &T = tables->T;
+    { const int rcd = check_device(tables); if (rcd != TJ_OK) return rcd; }
     g_prof.valid = false;   // set again when this call has recorded all of its events
     C.T = &T;
     C.nw = nw;
@@ -620,6 +667,7 @@ int run_coupling(const tj_tables *tables, int lcut, const double *d_Wtt, const d
 {
     if (use_small_path(tables->T, lcut, nw, spin)) {
         // single-launch path (tj_small.cu): no scratch, no tile list
+        { const int rcd = check_device(tables); if (rcd != TJ_OK) return rcd; }
         if ((d_TT && !d_Wtt) || (d_TE && !d_Wtp) || ((d_EE || d_BB || d_EB) && !d_Wpp)) return TJ_EINVAL;
         if (!d_TT && !d_TE && !d_EE && !d_BB && !d_EB) return TJ_EINVAL;
         const int mask = (!d_TE && !d_EE && !d_BB && !d_EB) ? M_TT : (d_TT ? M_TT : 0) | M_TE | M_EE | M_EB;
@@ -753,91 +801,100 @@ int run_literal(const tj_tables *tables, const double *d_Wtt, const double *d_Wp
 // copy loop) is copied to the host while chunk k+1 is computed.  Successive chunks alternate between two compute
 // streams so that one chunk's last CTAs overlap the next chunk's first ones; within a chunk the tiles keep the
 // descending (largest-first) order.
-struct HostPipe {
-    cudaStream_t comp[2] = {nullptr, nullptr}, copy = nullptr;
-    bool have = false;
-};
-thread_local HostPipe g_pipe;
-
 int run_coupling_rows_to_host(const tj_tables *tables, const double *d_Wtt, const double *d_Wtp, const double *d_Wpp,
                               int nW, double *const d_out[5], double *const h_out[5], cudaStream_t st)
 {
-    // chunk ends as fractions of the rows.  The device-to-host copies (rectangles with a row pitch: an effective
-    // ~35 GB/s here, where one contiguous copy reaches 54 GB/s, so 4 GB take ~115 ms against ~134 ms of compute at
-    // lmax = 10^4) must start early and never starve: a first chunk of 20 % of the rows is 10 %
-    // of the work, and with the L-shaped copies below it already releases 36 % of the bytes.  Measured end to end at
-    // config 3: 4 chunks 163 ms, 6 chunks 145 ms, 15 shrinking chunks 137.0 ms, these 10 chunks 135.4 ms
-    // (device-buffer call: 134.4 ms).
-    static const double kFrac[] = {0.20, 0.35, 0.47, 0.57, 0.66, 0.74, 0.81, 0.88, 0.94, 1.0};
-    constexpr int KMAX = (int)(sizeof(kFrac) / sizeof(kFrac[0]));
-    if (!g_pipe.have) {
-        for (int k = 0; k < 2; ++k) TJ_CUDA(cudaStreamCreateWithFlags(&g_pipe.comp[k], cudaStreamNonBlocking), "host pipe");
-        TJ_CUDA(cudaStreamCreateWithFlags(&g_pipe.copy, cudaStreamNonBlocking), "host pipe");
-        g_pipe.have = true;
-    }
+    HostPipe &pipe = const_cast<tj_tables *>(tables)->pipe;
+    std::lock_guard<std::mutex> lock(pipe.mu);
+    TJ_CUDA(pipe.ensure(), "host pipe");
     Call C;
     int rc = coupling_begin(C, tables, -1, d_Wtt, d_Wtp, d_Wpp, nW, d_out[0], d_out[1], d_out[2], d_out[3], d_out[4], st);
     if (rc != TJ_OK) return rc;
+
+    // Which regime?  Device-to-host copies reach ~54 GB/s when contiguous and ~35 GB/s as pitched rectangles (measured on
+    // this pool).  A call whose copies take longer than its arithmetic even at the contiguous rate is
+    // COPY-BOUND (config 2: 1.0 GB = 18.5 ms against 17.3 ms of compute): there every byte must move at the contiguous
+    // rate and the copy engine must never wait, so whole rows go out, chunk after chunk, in many small chunks (a row
+    // is final when its own chunk is done: its left part was mirrored there by the chunks above).  Otherwise the call
+    // is COMPUTE-BOUND (config 3: 74 ms of copies behind 134 ms of compute) and what matters is a short tail: after
+    // chunk k the L-shaped region it made final goes out (its rows from column r0 on, and columns [r0,r1) of all rows
+    // below), so that the last rows, cheap to compute but as long as any other, are nearly all on the host already.
+    int nmat_host = 0;
+    for (int m = 0; m < 5; ++m) nmat_host += h_out[m] ? 1 : 0;
+    const double copy_s = (double)nmat_host * (double)C.N * (double)C.N * 8.0 / 54e9;
+    const double n3 = (double)C.N * (double)C.N * (double)C.N / 6.0;   // even (and odd) steps of the upper triangle
+    const double comp_s = (C.mask == M_TT ? 2.0 : 13.0) * n3 / 1.6e13;
+    const bool rows_mode = copy_s > comp_s;
+    // chunk ends as fractions of the rows.  Compute-bound: a first chunk of 20 % of the rows is 10 % of the work and
+    // releases 36 % of the bytes (measured at config 3: 4 chunks 163 ms, 6 chunks 145 ms, these 10 chunks 135.4 ms;
+    // device-buffer call 134.4 ms).  Copy-bound: 1 % first (the copy engine starts at once), then even steps; measured
+    // at config 2 (floor: 1.0 GB at 54 GB/s = 18.5 ms): 8 chunks 25.9 ms, 13 chunks 22.2, 21 chunks 20.9, 24 chunks 20.5,
+    // 32 chunks 22.1, 48 chunks 23.8 (the L-shaped scheme of the compute-bound case: 24.5 ms).
+    static const double kFracL[] = {0.20, 0.35, 0.47, 0.57, 0.66, 0.74, 0.81, 0.88, 0.94, 1.0};
+    double frac[PIPE_MAX_CHUNKS];
+    int nfrac = 0;
+    if (rows_mode) {
+        frac[nfrac++] = 0.01;
+        for (int k = 1; k <= 22; ++k) frac[nfrac++] = 0.01 + 0.98 * k / 22.0;
+        frac[nfrac++] = 1.0;
+    } else {
+        for (double f : kFracL) frac[nfrac++] = f;
+    }
     // chunk boundaries: multiples of lcm(R, 32) rows (whole row bands of the sweep, whole tile rows of the writer)
     int L = C.R;
     while (L % 32) L += C.R;
-    int bound[KMAX + 1];
+    int bound[PIPE_MAX_CHUNKS + 1];
     int nchunk = 0;
     bound[0] = 0;
-    for (int k = 0; k < KMAX; ++k) {
-        long long r = (k == KMAX - 1) ? C.N : (long long)(kFrac[k] * (double)C.N) / L * L;
+    for (int k = 0; k < nfrac; ++k) {
+        long long r = (k == nfrac - 1) ? C.N : (long long)(frac[k] * (double)C.N) / L * L;
         if (r > bound[nchunk]) bound[++nchunk] = (int)r;
     }
-    cudaEvent_t ev[KMAX + 2];
-    int nev = 0;
-    cudaError_t e = cudaSuccess;
-    for (int k = 0; k < nchunk + 2 && e == cudaSuccess; ++k) {
-        e = cudaEventCreateWithFlags(&ev[k], cudaEventDisableTiming);
-        if (e == cudaSuccess) ++nev;
-    }
-    cudaEvent_t fork = ev[nchunk], join = ev[nchunk + 1];
-    if (e == cudaSuccess) e = cudaEventRecord(fork, st);
-    for (int k = 0; k < 2 && e == cudaSuccess; ++k) e = cudaStreamWaitEvent(g_pipe.comp[k], fork, 0);
-    if (e == cudaSuccess) e = cudaStreamWaitEvent(g_pipe.copy, fork, 0);
+    cudaEvent_t *ev = pipe.ev;
+    cudaEvent_t fork = ev[PIPE_MAX_CHUNKS], join = ev[PIPE_MAX_CHUNKS + 1];
+    cudaError_t e = cudaEventRecord(fork, st);
+    for (int k = 0; k < 2 && e == cudaSuccess; ++k) e = cudaStreamWaitEvent(pipe.comp[k], fork, 0);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(pipe.copy, fork, 0);
     for (int k = 0; k < nchunk && e == cudaSuccess; ++k) {
         const int r0 = bound[k], r1 = bound[k + 1];
-        cudaStream_t cs = g_pipe.comp[k & 1];
+        // successive chunks alternate between two compute streams: one chunk's last CTAs overlap the next one's first
+        cudaStream_t cs = pipe.comp[k & 1];
         const int b1 = (r1 == C.N) ? C.nb : r1 / C.R;
         const int I1 = (r1 == C.N) ? C.ntile_w : r1 / 32;
         e = coupling_sweep(C, r0 / C.R, b1, cs);
         if (e == cudaSuccess) e = coupling_write(C, r0 / 32, I1, cs);
         if (e == cudaSuccess) e = cudaEventRecord(ev[k], cs);
-        if (e == cudaSuccess) e = cudaStreamWaitEvent(g_pipe.copy, ev[k], 0);
-        if (e == cudaSuccess && k > 0) e = cudaStreamWaitEvent(g_pipe.copy, ev[k - 1], 0);
-        // What is final after chunk k: its own rows from column r0 on (their columns < r0 were final earlier), and,
-        // for every row BELOW the chunk, the columns [r0, r1) (the mirror of this chunk's bands).  Copying these two
-        // rectangles per chunk moves every element once and spreads the traffic evenly: the last rows, which are
-        // cheap to compute but as long as any other, have all but their last few columns on the host already.
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(pipe.copy, ev[k], 0);
+        if (e == cudaSuccess && k > 0) e = cudaStreamWaitEvent(pipe.copy, ev[k - 1], 0);
         const size_t pitch = sizeof(double) * (size_t)C.N;
         for (int m = 0; m < 5 && e == cudaSuccess; ++m) {
             if (!h_out[m]) continue;
             const double *src = d_out[m] ? d_out[m] : d_out[2];   // BB without its own device matrix: the EE rows
+            if (rows_mode) {
+                const size_t o = (size_t)r0 * (size_t)C.N;
+                e = cudaMemcpyAsync(h_out[m] + o, src + o, pitch * (size_t)(r1 - r0), cudaMemcpyDeviceToHost, pipe.copy);
+                continue;
+            }
             const size_t o1 = (size_t)r0 * (size_t)C.N + (size_t)r0;
             e = cudaMemcpy2DAsync(h_out[m] + o1, pitch, src + o1, pitch, sizeof(double) * (size_t)(C.N - r0),
-                                  (size_t)(r1 - r0), cudaMemcpyDeviceToHost, g_pipe.copy);
+                                  (size_t)(r1 - r0), cudaMemcpyDeviceToHost, pipe.copy);
             if (e == cudaSuccess && r1 < C.N) {
                 const size_t o2 = (size_t)r1 * (size_t)C.N + (size_t)r0;
                 e = cudaMemcpy2DAsync(h_out[m] + o2, pitch, src + o2, pitch, sizeof(double) * (size_t)(r1 - r0),
-                                      (size_t)(C.N - r1), cudaMemcpyDeviceToHost, g_pipe.copy);
+                                      (size_t)(C.N - r1), cudaMemcpyDeviceToHost, pipe.copy);
             }
         }
     }
-    // join: the caller's stream continues after everything issued above
-    if (nev == nchunk + 2) {
-        for (int k = 0; k < 2; ++k)
-            if (cudaEventRecord(join, g_pipe.comp[k]) == cudaSuccess) cudaStreamWaitEvent(st, join, 0);
-        if (cudaEventRecord(join, g_pipe.copy) == cudaSuccess) cudaStreamWaitEvent(st, join, 0);
-    } else {
-        cudaDeviceSynchronize();
+    // join: the caller's stream continues after everything issued above.  If anything failed on the way, wait for
+    // the whole device instead, so that no side stream still uses the scratch that is freed below.
+    bool joined = e == cudaSuccess;
+    for (int k = 0; k < 3 && joined; ++k) {
+        cudaStream_t s = k < 2 ? pipe.comp[k] : pipe.copy;
+        joined = cudaEventRecord(join, s) == cudaSuccess && cudaStreamWaitEvent(st, join, 0) == cudaSuccess;
     }
+    if (!joined) cudaDeviceSynchronize();
     if (e != cudaSuccess) rc = cuda_fail(e, "coupling/host pipeline");
     coupling_end(C, st);
-    for (int k = 0; k < nev; ++k) cudaEventDestroy(ev[k]);
     return rc;
 }
 
