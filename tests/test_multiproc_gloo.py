@@ -62,6 +62,61 @@ def test_window_set_sharding_and_timing_reduction_world2():
         assert len(set(flat)) == n_sets
 
 
+def _rows_worker(rank, world, port, lmax, q):
+    sys.path.insert(0, ROOT)
+    from paper_2602_15605_b200 import shard
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    N = lmax + 1
+    lo, hi = shard.row_blocks(lmax, world)[rank]
+    # entries this rank stores (tj_coupling_rows: full rows [lo, hi)), and the upper-triangle pairs it must sweep for
+    # them: (l1, l2 >= l1) with l1 in the block (direct) or l2 in the block (mirrored into row l2)
+    stored = torch.zeros((N, N), dtype=torch.int32)
+    stored[lo:hi, :] = 1
+    l1 = torch.arange(N)[:, None]
+    l2 = torch.arange(N)[None, :]
+    swept = ((l2 >= l1) & (((l1 >= lo) & (l1 < hi)) | ((l2 >= lo) & (l2 < hi)))).to(torch.int32)
+    tot_stored, tot_swept = stored.clone(), swept.clone()
+    dist.all_reduce(tot_stored)
+    dist.all_reduce(tot_swept)
+    work = torch.tensor([float(((torch.minimum(l1, l2) + 1) * swept).sum())], dtype=torch.float64)
+    works = [torch.zeros(1, dtype=torch.float64) for _ in range(world)]
+    dist.all_gather(works, work)
+    q.put((rank, (lo, hi), tot_stored, tot_swept, [float(w) for w in works]))
+    dist.destroy_process_group()
+
+
+def test_split_rows_blocks_tile_the_matrix_world2():
+    """bench.py --split-rows: the row blocks of the two ranks store every (l1,l2) exactly once; every upper-triangle
+    pair is swept by the owner(s) of its two rows (once on the diagonal blocks, twice across blocks); the sweep work
+    of the ranks is balanced."""
+    world, lmax = 2, 61
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_rows_worker, args=(r, world, port, lmax, q)) for r in range(world)]
+    for p in procs:
+        p.start()
+    res = [q.get(timeout=120) for _ in range(world)]
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    N = lmax + 1
+    blocks = sorted(r[1] for r in res)
+    assert blocks[0][0] == 0 and blocks[-1][1] == N and blocks[0][1] == blocks[1][0]
+    cut = blocks[0][1]
+    for rank, _, tot_stored, tot_swept, works in res:
+        assert bool((tot_stored == 1).all())                                   # each entry stored by exactly one rank
+        l1 = torch.arange(N)[:, None]
+        l2 = torch.arange(N)[None, :]
+        upper = l2 >= l1
+        cross = upper & (l1 < cut) & (l2 >= cut)                               # rows owned by different ranks
+        assert bool((tot_swept[upper & ~cross] == 1).all()) and bool((tot_swept[cross] == 2).all())
+        assert bool((tot_swept[~upper] == 0).all())
+        assert max(works) <= 1.15 * min(works)                                 # balanced (small N: coarse rows)
+
+
 def test_assign_window_sets_edge_cases():
     from paper_2602_15605_b200 import shard
     assert shard.assign_window_sets(0, 4, 1) == []
