@@ -24,25 +24,17 @@ constexpr int GUARD_HI = 768;
 // blockIdx alone, so ptxas keeps it in the uniform datapath instead of broadcasting five registers per bulk copy
 // (measured at config 3: 137.3 ms with 128 threads, 136.3 with 64, 133.5 with 32).
 constexpr int SWEEP_THREADS = 32;
-// (TJ_R_POL, TJ_TS_LONG/TJ_TS_SHORT/TJ_PIPE/TJ_MINB_POL and TJ_TS_BAND are tuning hooks: `TJ_NVCC_EXTRA="-DTJ_R_POL=14 ..." python -m
-// paper_2602_15605_b200.build --force` rebuilds with another geometry; the defaults are the measured optimum)
-#ifndef TJ_R_POL
-#define TJ_R_POL 12
-#endif
-constexpr int R_POL = TJ_R_POL;           // pairs per thread, fused TT+TE+EE(+EB) sweep, dense storage
-#ifndef TJ_R_BAND
-#define TJ_R_BAND 8
-#endif
-constexpr int R_POL_MID = 8;        // same at lmax < LMAX_MID: shorter sweeps, fewer tiles -- smaller tiles balance better (measured at lmax = 2000: 1.288 -> 1.230 ms per call)
+// (the geometry constants below are the measured optima)
+constexpr int R_POL = 12;           // pairs per thread, fused TT+TE+EE(+EB) sweep, dense storage, lmax >= LMAX_MID
+constexpr int R_POL_MID = 8;        // same at lmax < LMAX_MID: shorter sweeps, fewer tiles -- smaller tiles balance better
+                                    // (measured per call at lmax = 2000: R = 12 1.288 ms, 10 1.249, 8 1.227, 6 1.283)
 constexpr int LMAX_MID = 2600;
-constexpr int R_POL_BAND = TJ_R_BAND;       // same, band-limited (short sweeps)
+constexpr int R_POL_BAND = 8;       // same, band-limited (short sweeps)
 constexpr int R_TT = 16;            // pairs per thread, TT-only sweep (short sweeps)
 constexpr int R_TT_BAND = 16;       // same, band-limited
 constexpr int R_TT_LONG = 32;       // same, dense sweeps at lmax >= LMAX_LONG (measured at lmax = 10^4: 24.9 -> 22.8 ms)
-#ifndef TJ_LMAX_SMALL
-#define TJ_LMAX_SMALL 800
-#endif
-constexpr int LMAX_SMALL = TJ_LMAX_SMALL;   // up to here dense single-window calls take the single-launch path (tj_small.cu)
+constexpr int LMAX_SMALL = 800;     // up to here dense single-window calls take the single-launch path (tj_small.cu);
+                                    // measured crossover with the general path: all blocks 188 vs 207 us at 800, 317 vs 288 at 1000
 constexpr int LMAX_LONG = 4096;     // from here on a dense sweep uses the long-sweep geometry (R_TT_LONG; 96-step stages)
 constexpr int R_MULTI2 = 8;         // pairs per thread, 2 window sets per sweep (tj_coupling_multi)
 constexpr int R_MULTI3 = 6;         // pairs per thread, 3 window sets per sweep

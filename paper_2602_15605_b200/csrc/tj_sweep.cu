@@ -52,24 +52,13 @@
 namespace tj {
 namespace {
 
-// steps per stage of the dense polarised sweep (a multiple of R_POL, even): long stages amortise the stage
-// turn-over (measured at lmax = 10^4 with 4-warp CTAs: TS = 24 148.8 ms, 48 143.4 ms, 96 141.7 ms); short
-// sweeps keep the short stage (less shared memory, finer first/last stage)
-#ifndef TJ_TS_LONG
-#define TJ_TS_LONG 96
-#define TJ_TS_SHORT 48
-#define TJ_PIPE true
-#endif
-#ifndef TJ_MINB_POL
-#define TJ_MINB_POL 2
-#endif
-constexpr int TS_DENSE_LONG = TJ_TS_LONG, TS_DENSE_SHORT = TJ_TS_SHORT;
-#ifndef TJ_TS_BAND
-#define TJ_TS_BAND 64
-#endif
-#ifndef TJ_MINB_BAND
-#define TJ_MINB_BAND 3
-#endif
+// steps per stage (a multiple of R, even): long stages amortise the stage turn-over (measured at lmax = 10^4 with
+// 4-warp CTAs: TS = 24 148.8 ms, 48 143.4 ms, 96 141.7 ms; at lmax = 2000 96 is 1-1.6 % better than 48 as well, now
+// that the last stage is cut at the band's last block)
+constexpr int TS_DENSE = 96;      // dense polarised sweeps
+constexpr int TS_SPIN1 = 48;      // spin-1 sweeps (as measured in round 1)
+constexpr int TS_BAND = 64;       // band-limited sweeps (measured at config 4: 32: 0.3444 ms, 48: 0.3416, 64: 0.3417, 96: 0.3508)
+constexpr bool PIPE_DENSE = true; // TE/EE accumulations of step t issued at the start of step t+1
 constexpr int NBUF = 2;   // buffers per warp
 constexpr int PAD = 2;    // doubles in front of each slice: the software-pipelined read of "step TS" lands here
 
@@ -541,15 +530,15 @@ cudaError_t launch_sweep(const SweepParams &P, int mask, int nw, int spin, int t
         switch (mask) {
             case M_TT: return P.lmax >= LMAX_LONG ? launch_one<R_TT_LONG, M_TT, 64, 2, false, 1, 2, true>(P, total_tiles, st)
                                                   : launch_one<R_TT, M_TT, 48, 3, false, 1, 2, true>(P, total_tiles, st);
-            case POL: return launch_one<R_POL, POL, TS_DENSE_LONG, 2, TJ_PIPE, 1, 2, true>(P, total_tiles, st);
-            case ALL: return launch_one<R_POL, ALL, TS_DENSE_LONG, 2, TJ_PIPE, 1, 2, true>(P, total_tiles, st);
+            case POL: return launch_one<R_POL, POL, TS_DENSE, 2, PIPE_DENSE, 1, 2, true>(P, total_tiles, st);
+            case ALL: return launch_one<R_POL, ALL, TS_DENSE, 2, PIPE_DENSE, 1, 2, true>(P, total_tiles, st);
             default: return cudaErrorInvalidValue;
         }
     }
     if (spin == 1) {   // dense, one window set; TT-only requests use the spin-independent TT sweep below
         if (banded || nw != 1) return cudaErrorInvalidValue;
-        if (mask == ALL) return launch_one<R_POL, ALL, TS_DENSE_SHORT, 2, TJ_PIPE, 1, 1>(P, total_tiles, st);
-        if (mask == POL) return launch_one<R_POL, POL, TS_DENSE_SHORT, 2, TJ_PIPE, 1, 1>(P, total_tiles, st);
+        if (mask == ALL) return launch_one<R_POL, ALL, TS_SPIN1, 2, PIPE_DENSE, 1, 1>(P, total_tiles, st);
+        if (mask == POL) return launch_one<R_POL, POL, TS_SPIN1, 2, PIPE_DENSE, 1, 1>(P, total_tiles, st);
     }
     if (nw == 2 && !banded && mask == ALL) return launch_one<R_MULTI2, ALL, 48, 2, true, 2>(P, total_tiles, st);
     if (nw == 3 && !banded && mask == ALL) return launch_one<R_MULTI3, ALL, 36, 2, true, 3>(P, total_tiles, st);
@@ -562,13 +551,13 @@ cudaError_t launch_sweep(const SweepParams &P, int mask, int nw, int spin, int t
                           : (P.lmax >= LMAX_LONG ? launch_one<R_TT_LONG, M_TT, 64, 2, false>(P, total_tiles, st)
                                                  : launch_one<R_TT, M_TT, 48, 3, false>(P, total_tiles, st));
         case POL:
-            return banded ? launch_one<R_POL_BAND, POL, TJ_TS_BAND, TJ_MINB_BAND, false, 1, 2, false, true>(P, total_tiles, st)
-                          : (P.lmax >= LMAX_MID ? launch_one<R_POL, POL, TS_DENSE_LONG, TJ_MINB_POL, TJ_PIPE>(P, total_tiles, st)
-                                                       : launch_one<R_POL_MID, POL, TS_DENSE_LONG, 2, TJ_PIPE>(P, total_tiles, st));
+            return banded ? launch_one<R_POL_BAND, POL, TS_BAND, 3, false, 1, 2, false, true>(P, total_tiles, st)
+                          : (P.lmax >= LMAX_MID ? launch_one<R_POL, POL, TS_DENSE, 2, PIPE_DENSE>(P, total_tiles, st)
+                                                       : launch_one<R_POL_MID, POL, TS_DENSE, 2, PIPE_DENSE>(P, total_tiles, st));
         case ALL:
-            return banded ? launch_one<R_POL_BAND, ALL, TJ_TS_BAND, TJ_MINB_BAND, false, 1, 2, false, true>(P, total_tiles, st)
-                          : (P.lmax >= LMAX_MID ? launch_one<R_POL, ALL, TS_DENSE_LONG, TJ_MINB_POL, TJ_PIPE>(P, total_tiles, st)
-                                                       : launch_one<R_POL_MID, ALL, TS_DENSE_LONG, 2, TJ_PIPE>(P, total_tiles, st));
+            return banded ? launch_one<R_POL_BAND, ALL, TS_BAND, 3, false, 1, 2, false, true>(P, total_tiles, st)
+                          : (P.lmax >= LMAX_MID ? launch_one<R_POL, ALL, TS_DENSE, 2, PIPE_DENSE>(P, total_tiles, st)
+                                                       : launch_one<R_POL_MID, ALL, TS_DENSE, 2, PIPE_DENSE>(P, total_tiles, st));
         default: return cudaErrorInvalidValue;
     }
 }
