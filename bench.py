@@ -389,16 +389,20 @@ def main():
     else:
         alg_instr = INSTR_EVEN_TT * E
         alg_flops = 3 * E
+    unbatched_equiv = None
     if nwin > 1:
-        # the per-kernel events cover the LAST sweep of the call (one pair of window sets, or a single set when
-        # nwin is odd); algorithmic work is counted as for the unbatched method: (8E+5O) per window set
-        left, ngroups = nwin, 0
-        while left > 0:        # the library's grouping: threes, a remainder of 4 as 2 + 2, of 2 as one pair
+        # the per-kernel events cover the LAST sweep of the call (the library's grouping: threes, a remainder of 4 as
+        # 2 + 2, of 2 as one pair).  A batched sweep forms the window-independent part of a term once:
+        # 5 + 3 nw instructions per even term and 4 + nw per odd term for nw window sets; that is the algorithmic work of
+        # the launch.  The work the UNBATCHED method would need for the same matrices ((8E+5O) per window set) is
+        # reported beside it as `unbatched_equivalent_frac` (it may exceed 1: that is the point of batching).
+        left = nwin
+        while left > 0:
             last = 2 if left in (2, 4) else 3 if left >= 3 else 1
             left -= last
-            ngroups += 1
-        alg_instr *= last
-        alg_flops *= last
+        unbatched_equiv = alg_instr * last
+        alg_instr = (5 + 3 * last) * E + (4 + last) * O
+        alg_flops = (6 + 6 * last) * E + (4 + 2 * last) * O
     peaks, peak_kind = _peaks()
     traffic, traffic_src = _traffic(wl.name if nwin == 1 and not split else None, geo)
     sm_max = float(clocks.get("sm_max_mhz") or peaks.get("sm_max_mhz", 1965.0))
@@ -430,6 +434,7 @@ def main():
                        % (SM_COUNT, FP64_LANES_PER_SM, sm_max),
         "algorithmic_instr_per_launch": alg_instr, "algorithmic_flops_per_launch": alg_flops,
         "achieved_tflops": alg_flops / (sweep_ms * 1e-3) / 1e12,
+        "unbatched_equivalent_frac": None if unbatched_equiv is None else unbatched_equiv / (sweep_ms * 1e-3) / peak_instr,
         "measured_dfma_peak": probe / 1e12, "frac_of_measured_dfma": achieved / probe,
         "dfma_probe": {"seconds": probe_s, "iterations": it, "sm_mhz": probe_clocks.get("sm_mhz"),
                        "reasons": probe_clocks.get("reasons"), "power_w_max": probe_clocks.get("power_w_max")},
