@@ -977,3 +977,58 @@ def test_binned_flat_window_closed_form_multi_chunk():
     pol[:, 0] = 0.0                                   # bin 0 = l < 2
     assert np.all(np.abs(B["EE"] + B["EB"] - pol) <= 1e-11 * np.maximum(want, 1e-30))
     T.close()
+
+
+# ---------------------------------------------------------------- sizes far past the configs (index arithmetic, table range)
+def test_flat_window_closed_form_tt_lmax40000():
+    """The largest dense size the tests run: lmax = 40000 (TT alone: 12.8 GB, tables up to p = 80001, 2.0e6 one-warp
+    tiles): the flat-window closed form K^TT = (2 l2+1)/(4 pi) (orthogonality over l3) in every entry."""
+    import torch
+    lmax = 40000
+    N = lmax + 1
+    free, _ = torch.cuda.mem_get_info()
+    if free < 16 * 2 ** 30:
+        pytest.skip("needs 16 GB of free device memory")
+    W = _t(windows.flat(2 * lmax))
+    T = binding.build_tables(lmax)
+    TT = binding.coupling_tt(T, W)
+    torch.cuda.synchronize()
+    col = (2.0 * torch.arange(N, dtype=torch.float64, device="cuda") + 1.0) / (4 * math.pi)
+    worst = 0.0
+    for r0 in range(0, N, 4000):   # row chunks: no second matrix-sized temporary
+        blk = TT[r0:r0 + 4000]
+        worst = max(worst, float(((blk - col[None, :]).abs() / col[None, :]).max()))
+    print("flat window lmax=40000: TT rel %.2e" % worst)
+    assert worst < 1e-12, worst
+    del TT
+    T.close()
+
+
+def test_band_long_matrix_lmax100000_lcut64_sampled():
+    """A band-limited call on a very long matrix (lmax = 10^5, L_cut = 64; 3126 diagonal blocks): every slot written,
+    out-of-range slots exactly 0, sampled entries against the oracle (which recurses the whole l3 range of each pair)."""
+    import torch
+    lmax, lcut = 100000, 64
+    l = np.arange(lcut + 1, dtype=np.float64)
+    W = 4.0 * math.pi * 0.25 * np.exp(-l * l / (2.0 * 20.0 ** 2))
+    Wtp = W * (1.0 - 0.01 * l)          # three different windows, TP with a sign change at l = 100 (none here) ...
+    Wpp = W * (1.0 + 0.02 * l)
+    T = binding.build_tables(lmax)
+    N, width = lmax + 1, 2 * lcut + 1
+    pre = {k: torch.full((N, width), float("nan"), dtype=torch.float64, device="cuda") for k in BLOCKS}
+    out = binding.coupling_band(T, lcut, _t(W), _t(Wtp), _t(Wpp), out=pre)
+    torch.cuda.synchronize()
+    l2grid = torch.arange(N, device="cuda")[:, None] + torch.arange(-lcut, lcut + 1, device="cuda")[None, :]
+    outside = (l2grid < 0) | (l2grid > lmax)
+    for k in BLOCKS:
+        assert bool(torch.isfinite(out[k]).all()), k
+        assert bool((out[k][outside] == 0).all()), k
+    assert bool((out["BB"] == out["EE"]).all())
+    l1, l2 = _sample_pairs(lmax, 300, 777, band=lcut)
+    ref = oracle.coupling_pairs(lcut, W, Wtp, Wpp, l1, l2)
+    i1 = torch.as_tensor(l1.astype(np.int64)).cuda()
+    io = torch.as_tensor((l2.astype(np.int64) - l1 + lcut)).cuda()
+    for k in BLOCKS:
+        got = out[k][i1, io].cpu().numpy()
+        assert_parity(got, ref[k], "band lmax=1e5 %s" % k)
+    T.close()
