@@ -408,15 +408,16 @@ def main():
     sm_max = float(clocks.get("sm_max_mhz") or peaks.get("sm_max_mhz", 1965.0))
     peak_instr = SM_COUNT * FP64_LANES_PER_SM * sm_max * 1e6          # thread-instr/s at max boost
     achieved = alg_instr / (sweep_ms * 1e-3)
-    # measured DFMA rate: a register-resident chain kernel on every SM for >= 1 s, clocks sampled
+    # measured DFMA rate (bench_gpu/fp64_probe.cu, bench-only): a register-resident chain kernel on every SM for >= 1 s, clocks sampled
     it = 2000000
-    rate = binding.fp64_probe(it)
+    import bench_gpu
+    rate = bench_gpu.fp64_probe(it)
     it = int(min(2.0e9, 1.15 * it * rate / (16.0 * it * SM_COUNT * 4 * 256)))   # iterations for ~1.15 s at that rate
     psampler = ClockSampler(local_rank)
     psampler.start()
     time.sleep(0.2)
     tp0 = time.perf_counter()
-    probe = binding.fp64_probe(it)
+    probe = bench_gpu.fp64_probe(it)
     probe_s = time.perf_counter() - tp0
     probe_clocks = psampler.stop()
     bytes_out = len(blocks) * N * width * 8

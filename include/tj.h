@@ -204,13 +204,6 @@ int tj_l3_range(int l1, int l2, int l3max, int parity, int *l3_lo, int *l3_hi, i
 int tj_sweep_counts(int l1, int l2, int l3max, int *te_lo, int *te_hi, int *to_lo, int *to_hi);
 
 /*
- * tj_fp64_probe -- measurement aid for the roofline denominator: runs `iters` dependent-chain DFMA
- * iterations of 16 independent chains per thread on every SM and returns, through *h_thread_instr_per_s,
- * the achieved FP64 thread-instructions per second (synchronous; CUDA-event timed).
- */
-int tj_fp64_probe(int iters, void *cuda_stream, double *h_thread_instr_per_s);
-
-/*
  * Per-kernel timing for the roofline (bench.py): while enabled, every coupling call records CUDA events
  * on its stream around its three kernels.  tj_profile_get waits for the most recent call made by the
  * calling thread and returns the device time in milliseconds of  h_ms3[0] prepare (a2+a3),

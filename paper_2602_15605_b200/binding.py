@@ -19,7 +19,7 @@ TJ_OK, TJ_EINVAL, TJ_ENOMEM, TJ_ECUDA = 0, -1, -2, -3
 SYMBOLS = (
     "tj_build_tables", "tj_free_tables", "tj_tables_info", "tj_tables_copy",
     "tj_coupling_tt", "tj_coupling_pol", "tj_coupling_band", "tj_coupling_multi", "tj_coupling_spin1", "tj_coupling_rows", "tj_coupling_binned", "tj_coupling_literal", "tj_coupling_host",
-    "tj_l3_range", "tj_sweep_counts", "tj_fp64_probe", "tj_profile_enable", "tj_profile_get",
+    "tj_l3_range", "tj_sweep_counts", "tj_profile_enable", "tj_profile_get",
     "tj_profile_last_sweep", "tj_profile_launches", "tj_strerror",
 )
 
@@ -60,7 +60,6 @@ def load_library() -> ctypes.CDLL:
     L.tj_coupling_host.argtypes = [vp, ci, ci, vp, vp, vp, vp, vp, vp, vp, vp, vp]
     L.tj_l3_range.argtypes = [ci, ci, ci, ci, ip, ip, ip]
     L.tj_sweep_counts.argtypes = [ci, ci, ci, ip, ip, ip, ip]
-    L.tj_fp64_probe.argtypes = [ci, vp, dp]
     L.tj_profile_enable.argtypes = [ci]
     L.tj_profile_get.argtypes = [dp]
     L.tj_profile_last_sweep.argtypes = [ip]
@@ -321,12 +320,6 @@ def sweep_counts(l1, l2, l3max):
     _check(load_library().tj_sweep_counts(l1, l2, l3max, ctypes.byref(a), ctypes.byref(b), ctypes.byref(c), ctypes.byref(d)),
            "tj_sweep_counts")
     return a.value, b.value, c.value, d.value
-
-
-def fp64_probe(iters=20000, stream=None):
-    v = ctypes.c_double()
-    _check(load_library().tj_fp64_probe(int(iters), _stream_ptr(stream), ctypes.byref(v)), "tj_fp64_probe")
-    return v.value
 
 
 def profile_launches() -> int:

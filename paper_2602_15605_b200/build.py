@@ -9,7 +9,7 @@ import sys
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 SO = os.path.join(_HERE, "libtj.so")
-SOURCES = ["tj_api.cu", "tj_tables.cu", "tj_prepare.cu", "tj_sweep.cu", "tj_writer.cu", "tj_probe.cu", "tj_literal.cu", "tj_small.cu", "tj_binned.cu"]
+SOURCES = ["tj_api.cu", "tj_tables.cu", "tj_prepare.cu", "tj_sweep.cu", "tj_writer.cu", "tj_literal.cu", "tj_small.cu", "tj_binned.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "--fmad=true", "-Xcompiler", "-fPIC", "-Xcompiler", "-O2"]
 

@@ -433,37 +433,6 @@ int tj_sweep_counts(int l1, int l2, int l3max, int *te_lo, int *te_hi, int *to_l
     return TJ_OK;
 }
 
-int tj_fp64_probe(int iters, void *cuda_stream, double *h_thread_instr_per_s)
-{
-    if (iters <= 0 || !h_thread_instr_per_s) return TJ_EINVAL;
-    cudaStream_t st = (cudaStream_t)cuda_stream;
-    int dev = 0, sms = 0;
-    TJ_CUDA(cudaGetDevice(&dev), "tj_fp64_probe");
-    TJ_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev), "tj_fp64_probe");
-    const int threads = 256, blocks = sms * 4;
-    double *sink = nullptr;
-    TJ_CUDA(cudaMalloc((void **)&sink, sizeof(double) * (size_t)blocks * threads), "tj_fp64_probe/alloc");
-    cudaEvent_t e0, e1;
-    cudaEventCreate(&e0);
-    cudaEventCreate(&e1);
-    cudaError_t e = launch_fp64_probe(iters / 8 + 1, sink, blocks, threads, st);  // warm-up
-    cudaEventRecord(e0, st);
-    if (e == cudaSuccess) e = launch_fp64_probe(iters, sink, blocks, threads, st);
-    cudaEventRecord(e1, st);
-    cudaError_t es = cudaEventSynchronize(e1);
-    float ms = 0.f;
-    cudaEventElapsedTime(&ms, e0, e1);
-    cudaEventDestroy(e0);
-    cudaEventDestroy(e1);
-    cudaFree(sink);
-    if (e != cudaSuccess) return cuda_fail(e, "tj_fp64_probe/launch");
-    if (es != cudaSuccess) return cuda_fail(es, "tj_fp64_probe/sync");
-    // 16 DFMA per loop iteration per thread
-    const double instr = 16.0 * (double)iters * (double)blocks * (double)threads;
-    *h_thread_instr_per_s = instr / ((double)ms * 1e-3);
-    return TJ_OK;
-}
-
 int tj_profile_enable(int on)
 {
     g_profile.store(on ? 1 : 0);
@@ -610,7 +579,6 @@ cudaError_t coupling_sweep(const Call &C, int b0, int b1, cudaStream_t st)
     const bool all = (b0 == 0 && b1 == C.nb);
     P.tile_off = all ? 0 : tiles_above(C, b1 - 1);
     P.wstride = WSET * (long long)T.nl_alloc;
-    P.even_mask = ~1;
     P.row_lo = C.row_lo; P.row_hi = C.row_hi; P.rows = C.rows ? 1 : 0;
     P.ostride = C.N * C.ld;
     const int n = all ? C.ntiles : tiles_above(C, b0 - 1) - P.tile_off;

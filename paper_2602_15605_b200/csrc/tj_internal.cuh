@@ -114,7 +114,6 @@ struct SweepParams {
     double *TT, *TE, *EE, *EB;      // raw Xi, upper triangle (dense: [l1*ld+l2]; band: [l1*ld + l2-l1+lcut])
     const int *tile_start;          // [nbands+1] exclusive prefix of tiles per band, bands in DESCENDING order
     int lmax, l3max, nbands, lcut;  // lcut < 0: dense storage
-    int even_mask;                  // ~1 (see the sweep: keeps a parity out of the compiler's sight)
     int row_lo, row_hi;             // full rows [row_lo, row_hi) are computed (whole matrix: 0, lmax+1)
     int rows;                       // 1: compact row-block outputs [(l1-row_lo)*ld + l2], direct AND mirrored entries stored
     int tile_off;                   // first tile of this launch in the descending-band prefix (row-chunked launches)
@@ -176,6 +175,5 @@ cudaError_t launch_small(const Tables &T, int mask, const double *d_Wtt, const d
                          double *TT, double *TE, double *EE, double *BB, double *EB, cudaStream_t st);
 cudaError_t launch_literal(const Tables &T, const double *wtt, const double *wpp, double *TT, double *EE, int l3max,
                            cudaStream_t st);   // paper-literal ablation kernel (tj_literal.cu)
-cudaError_t launch_fp64_probe(int iters, double *d_sink, int blocks, int threads, cudaStream_t st);
 
 }  // namespace tj

@@ -190,8 +190,9 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB * (128 / SWEEP_THREADS)) s
     const int t_end = a + R - 1;   // last step any pair of the band can have
     int tbo = sw - 1 - P.l3max;    // odd:  l3 = s-2t-1 <= l3max
     // first steps rounded down to even (an extra step adds exact zeros): the step factor g[t] is then read two steps
-    // per 16-byte load.  The mask is a kernel argument (always ~1) so that the compiler can NOT prove the parity and
-    // pair the row-ring loads too: those go into fixed ring registers and a paired load costs two register moves.
+    // per 16-byte load.  The result is then passed through an empty asm statement, so that the compiler can NOT prove
+    // its parity and pair the row-ring loads too: those go into fixed ring registers and a paired load costs two
+    // register moves.
     // Diagonal tiling: lane j starts j steps after lane 0, so lane 0 may start below 0 (the guard band of g[t] adds
     // exact zeros there) but not below -32: then every lane starts at or below its own first step max(0, .).
     // Then the first step moves further down so that the walk is whole blocks of R steps ENDING at the last step
@@ -205,8 +206,9 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB * (128 / SWEEP_THREADS)) s
         tbe = max((tbe + 1) >> 1, -32);
         tbe = t_end + 1 - R * ((t_end - tbe + R) / R);
     } else {
-        tbo = tbo > 0 ? ((tbo + 1) >> 1) & P.even_mask : 0;
-        tbe = tbe > 0 ? ((tbe + 1) >> 1) & P.even_mask : 0;
+        tbo = tbo > 0 ? ((tbo + 1) >> 1) & ~1 : 0;
+        tbe = tbe > 0 ? ((tbe + 1) >> 1) & ~1 : 0;
+        asm("" : "+r"(tbo), "+r"(tbe));   // opaque to the optimiser from here on (see above)
     }
     const int nso = (kEB && tbo <= t_end_o) ? (t_end_o - tbo + TS) / TS : 0;
     const int nse = (kEven && tbe <= t_end) ? (t_end - tbe + TS) / TS : 0;
