@@ -364,6 +364,25 @@ def test_full_size_configs_sampled(cfg, npairs):
     T.close()
 
 
+def _assert_band_row_sums(out, lmax, lcut, Wtt, Wpp, what):
+    """A property that needs no oracle and holds at any size (orthogonality of the 3j symbols over the third l at fixed
+    m's): in a band-limited matrix every row l1 with lcut <= l1 <= lmax-lcut holds its whole triangle,
+    so  sum_l2 K^TT = sum_l3 (2 l3+1) W^TT_l3 / 4 pi  and  sum_l2 (K^EE + K^EB) = the same with W^PP (l1 >= 2).
+    (TE has no such sum rule: its two symbols carry different m on l2.)  Pinned on the oracle in
+    tests/test_oracle_coupling.py::test_band_row_sum_rule."""
+    import torch
+    l3 = np.arange(lcut + 1, dtype=np.float64)
+    ctt = float(((2 * l3 + 1) * Wtt).sum() / (4 * math.pi))
+    cpp = float(((2 * l3 + 1) * Wpp).sum() / (4 * math.pi))
+    rows = slice(max(lcut, 2), lmax - lcut + 1)
+    stt = out["TT"][rows].sum(dim=1)
+    spp = out["EE"][rows].sum(dim=1) + out["EB"][rows].sum(dim=1)
+    e_tt = float((stt - ctt).abs().max() / ctt)
+    e_pp = float((spp - cpp).abs().max() / cpp)
+    print("%s: row sums over %d rows: TT %.2e, EE+EB %.2e" % (what, stt.numel(), e_tt, e_pp))
+    assert e_tt < 1e-12 and e_pp < 1e-12, (e_tt, e_pp)
+
+
 def test_cfg4_band_full_size_sampled():
     import torch
     wl = windows.config(4)
@@ -389,6 +408,7 @@ def test_cfg4_band_full_size_sampled():
         assert_parity(got, ref[k], "cfg4 %s" % k)
     # rows 0 and lmax: out-of-range slots zero
     assert torch.all(out["TT"][0, :lcut] == 0) and torch.all(out["TT"][-1, lcut + 1:] == 0)
+    _assert_band_row_sums(out, wl.lmax, lcut, wl.Wtt, wl.Wpp, "cfg4")
     T.close()
 
 
@@ -1031,4 +1051,5 @@ def test_band_long_matrix_lmax100000_lcut64_sampled():
     for k in BLOCKS:
         got = out[k][i1, io].cpu().numpy()
         assert_parity(got, ref[k], "band lmax=1e5 %s" % k)
+    _assert_band_row_sums(out, lmax, lcut, W, Wpp, "band lmax=1e5")
     T.close()

@@ -159,3 +159,23 @@ def test_windows_recipe_is_seeded_and_shaped():
             O += no
             P += 1 if ne + no > 0 else 0
     assert windows.term_counts(lmax, l3max) == (E, O, P)
+
+
+def test_band_row_sum_rule():
+    """Orthogonality over the third l at fixed m's (sum_l2 (2 l2+1) (l1 l2 l3; m1 m2 m3)^2 = 1): a row of a band-limited
+    matrix that holds its whole triangle (lcut <= l1 <= lmax-lcut) sums to sum_l3 (2 l3+1) W_l3 / 4 pi, for TT with W^TT
+    and for EE+EB with W^PP (l1 >= 2), whatever the window -- signed windows included.  (TE has no such rule.)"""
+    lmax, lcut = 60, 9
+    l = np.arange(lcut + 1, dtype=np.float64)
+    Wtt = np.exp(-l * l / 20.0) * (1.0 - 0.3 * l)       # changes sign at l = 4
+    Wpp = np.cos(0.7 * l) + 0.2
+    Wtp = 0.5 * Wtt + 0.1
+    r = oracle.coupling_band(lmax, lcut, Wtt, Wtp, Wpp)
+    c = lambda w: float(((2 * l + 1) * w).sum() / (4 * math.pi))   # noqa: E731
+    rows = slice(max(lcut, 2), lmax - lcut + 1)
+    scale = float(((2 * l + 1) * np.abs(Wtt)).sum() / (4 * math.pi))
+    assert np.abs(r["TT"][rows].sum(1) - c(Wtt)).max() < 1e-13 * scale
+    scale = float(((2 * l + 1) * np.abs(Wpp)).sum() / (4 * math.pi))
+    assert np.abs((r["EE"] + r["EB"])[rows].sum(1) - c(Wpp)).max() < 1e-13 * scale
+    # a row that does NOT hold its whole triangle falls short (the rule is not vacuous)
+    assert abs(r["TT"][lmax].sum() - c(Wtt)) > 1e-3 * scale
