@@ -565,6 +565,7 @@ cudaError_t coupling_sweep(const Call &C, int b0, int b1, cudaStream_t st)
     P.wtt = C.wtt; P.wtp = C.wtp; P.wpp = C.wpp; P.wA = C.wA; P.wB = C.wB;
     // a block the instantiated sweep computes but the caller did not ask for has a NULL target and is not stored
     P.TT = C.TT; P.TE = C.TE; P.EE = C.ee; P.EB = C.EB;
+    P.BB = C.rows ? C.bb_copy : nullptr;
     P.tile_start = C.tile_start;
     P.lmax = T.lmax; P.l3max = C.l3max_eff; P.nbands = C.nb; P.lcut = C.banded ? C.lcut : -1; P.ld = C.ld;
     P.nd = diag_num_blocks(T.lmax, C.R);
@@ -667,15 +668,6 @@ int run_rows(const tj_tables *tables, const double *d_Wtt, const double *d_Wtp, 
     prof_record(2, st);
     cudaError_t e = coupling_sweep(C, 0, C.nb, st);
     prof_record(3, st);
-    if (e == cudaSuccess) {
-        double *M[4] = {nullptr, nullptr, nullptr, nullptr};
-        int n = 0, bb_src = -1;
-        if (C.TT) M[n++] = C.TT;
-        if (C.TE) M[n++] = C.TE;
-        if (C.ee) { if (C.bb_copy) bb_src = n; M[n++] = C.ee; }
-        if (C.EB) M[n++] = C.EB;
-        e = launch_scale_rows(M, n, C.bb_copy, bb_src, (long long)(row_hi - row_lo), C.T->lmax, st);
-    }
     prof_record(4, st);
     if (e != cudaSuccess) rc = cuda_fail(e, "tj_coupling_rows");
     coupling_end(C, st);

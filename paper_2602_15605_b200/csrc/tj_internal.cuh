@@ -111,7 +111,9 @@ struct SweepParams {
     const double *g, *ginv, *h, *gA, *gB, *u3, *isd;
     const double *wtt, *wtp, *wpp;  // prefolded windows W'_X[l] = (2l+1) W_X[l] / (4 pi), pointer to l = 0
     const double *wA, *wB;          // the same as pairs: wA[2l..] = (W'_TT, W'_TP)[l], wB[2l..] = (W'_PP, u_l)[l]
-    double *TT, *TE, *EE, *EB;      // raw Xi, upper triangle (dense: [l1*ld+l2]; band: [l1*ld + l2-l1+lcut])
+    double *TT, *TE, *EE, *EB;      // raw Xi, upper triangle [l1*ld+l2]; band-limited calls: transposed scratch [delta*ld + l1];
+                                    // row blocks: the final K, direct and mirrored entries
+    double *BB;                     // row blocks: receives the EE values as well (NULL: none)
     const int *tile_start;          // [nbands+1] exclusive prefix of tiles per band, bands in DESCENDING order
     int lmax, l3max, nbands, lcut;  // lcut < 0: dense storage
     int row_lo, row_hi;             // full rows [row_lo, row_hi) are computed (whole matrix: 0, lmax+1)
@@ -163,8 +165,6 @@ cudaError_t launch_build_tables(const Tables &T, cudaStream_t st);
 cudaError_t launch_prepare(const Tables &T, const double *d_Wtt, const double *d_Wtp, const double *d_Wpp, int nW,
                            double *wtt, double *wtp, double *wpp, double *wA, double *wB, int *tile_start, int R,
                            int l3max_eff, bool banded, int row_lo, int row_hi, cudaStream_t st);
-// row-block outputs: M[r][c] *= (2c+1) for the nmat blocks in M (rows x (lmax+1) each), bb = copy of M[bb_src] or NULL
-cudaError_t launch_scale_rows(double *const M[4], int nmat, double *bb, int bb_src, long long rows, int lmax, cudaStream_t st);
 int sweep_R(int mask, bool banded, int nw, int lmax, bool rows, int spin);   // pairs per thread (= rows per band) of the sweep that serves `mask` for nw window sets
 cudaError_t launch_sweep(const SweepParams &P, int mask, int nw, int spin, int total_tiles, cudaStream_t st);
 cudaError_t launch_writer(const WriterParams &P, cudaStream_t st);

@@ -351,10 +351,12 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB * (128 / SWEEP_THREADS)) s
                     for (int w = 0; w < NW; ++w)
                         P.EB[w * P.ostride + idx] = acc[w][i] * (0.25 * sd * sd);
                 }
-                if (P.EB && ROWS) {   // row block: Xi(l1,l2) goes to [l1][l2] and, mirrored, to [l2][l1], where inside
+                if (P.EB && ROWS) {
+                    // row block: a block of full rows has no in-place triangle to mirror, so the final values are stored
+                    // here: K = (2 l2+1) Xi at [l1][l2] and (2 l1+1) Xi at [l2][l1], where inside
                     const double v = acc[0][i] * (0.25 * sd * sd);
-                    if (l1 >= P.row_lo && l1 < P.row_hi) P.EB[(long long)(l1 - P.row_lo) * P.ld + l2] = v;
-                    if (l2 >= P.row_lo && l2 < P.row_hi && l2 != l1) P.EB[(long long)(l2 - P.row_lo) * P.ld + l1] = v;
+                    if (l1 >= P.row_lo && l1 < P.row_hi) P.EB[(long long)(l1 - P.row_lo) * P.ld + l2] = v * (double)(2 * l2 + 1);
+                    if (l2 >= P.row_lo && l2 < P.row_hi && l2 != l1) P.EB[(long long)(l2 - P.row_lo) * P.ld + l1] = v * (double)(2 * l1 + 1);
                 }
             }
         }
@@ -476,9 +478,14 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB * (128 / SWEEP_THREADS)) s
                 } else {   // row block (see the odd branch)
                     const bool in1 = l1 >= P.row_lo && l1 < P.row_hi, in2 = l2 >= P.row_lo && l2 < P.row_hi && l2 != l1;
                     const long long i1 = (long long)(l1 - P.row_lo) * P.ld + l2, i2 = (long long)(l2 - P.row_lo) * P.ld + l1;
-                    if (kTT && P.TT) { const double v = att[0][i]; if (in1) P.TT[i1] = v; if (in2) P.TT[i2] = v; }
-                    if (kTE && P.TE) { const double v = ate[0][i] * (0.5 * sd); if (in1) P.TE[i1] = v; if (in2) P.TE[i2] = v; }
-                    if (kEE && P.EE) { const double v = aee[0][i] * (0.25 * sd * sd); if (in1) P.EE[i1] = v; if (in2) P.EE[i2] = v; }
+                    const double w2 = (double)(2 * l2 + 1), w1 = (double)(2 * l1 + 1);   // K = (2 l2+1) Xi; mirrored: (2 l1+1) Xi
+                    if (kTT && P.TT) { const double v = att[0][i]; if (in1) P.TT[i1] = v * w2; if (in2) P.TT[i2] = v * w1; }
+                    if (kTE && P.TE) { const double v = ate[0][i] * (0.5 * sd); if (in1) P.TE[i1] = v * w2; if (in2) P.TE[i2] = v * w1; }
+                    if (kEE && P.EE) {
+                        const double v = aee[0][i] * (0.25 * sd * sd);
+                        if (in1) { P.EE[i1] = v * w2; if (P.BB) P.BB[i1] = v * w2; }   // BB beside EE
+                        if (in2) { P.EE[i2] = v * w1; if (P.BB) P.BB[i2] = v * w1; }
+                    }
                 }
             }
         }

@@ -93,35 +93,7 @@ __global__ void __launch_bounds__(WT * WROWS) writer_kernel(const __grid_constan
     }
 }
 
-// row-block outputs (tj_coupling_rows): the sweep stored Xi in both positions; K = (2 l2+1) Xi rides on the column
-__global__ void __launch_bounds__(256) scale_rows_kernel(double *m0, double *m1, double *m2, double *m3, int nmat, double *bb,
-                                                         int bb_src, long long total, int N)
-{
-    double *M[4] = {m0, m1, m2, m3};
-    for (long long ix = (long long)blockIdx.x * 256 + threadIdx.x; ix < total; ix += (long long)gridDim.x * 256) {
-        const double f = (double)(2 * (int)(ix % N) + 1);
-#pragma unroll
-        for (int m = 0; m < 4; ++m) {
-            if (m >= nmat) break;
-            const double v = M[m][ix] * f;
-            M[m][ix] = v;
-            if (bb != nullptr && m == bb_src) bb[ix] = v;
-        }
-    }
-}
-
 }  // namespace
-
-cudaError_t launch_scale_rows(double *const M[4], int nmat, double *bb, int bb_src, long long rows, int lmax, cudaStream_t st)
-{
-    if (nmat <= 0 || rows <= 0) return cudaSuccess;
-    const long long total = rows * ((long long)lmax + 1);
-    long long nb = (total + 255) / 256;
-    if (nb > 148 * 32) nb = 148 * 32;
-    scale_rows_kernel<<<(unsigned)nb, 256, 0, st>>>(M[0], M[1], M[2], M[3], nmat, bb, bb_src, total, lmax + 1);
-    ++g_launch_count;
-    return cudaGetLastError();
-}
 
 // One CTA: deltas d0..d0+31 of ONE banded output, and
 //   direct:  rows l1 = r0..r0+31:       M[l1][lcut+delta] = (2(l1+delta)+1) Xi(l1, l1+delta)   source X[delta][l1]
