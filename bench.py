@@ -218,6 +218,8 @@ def main():
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json configs index (headline: 3)")
     ap.add_argument("--nwin", type=int, default=1,
                     help="window sets per step through tj_coupling_multi (default 1: the headline tj_coupling_pol step)")
+    ap.add_argument("--tt-only", action="store_true",
+                    help="time tj_coupling_tt (K^TT alone, 2 FP64 instructions per term) on the config's W^TT instead of all five blocks")
     ap.add_argument("--split-rows", action="store_true",
                     help="N > 1: cut ONE matrix set into N work-balanced row blocks, one per rank (tj_coupling_rows, no "
                          "exchange; strong scaling) instead of one independent window set per rank (the default, weak)")
@@ -252,8 +254,11 @@ def main():
     binding.load_library()   # fails loudly if the CUDA library is missing: no fallback
 
     base = windows.config(args.config)
+    if args.tt_only and base.pol and not base.band:
+        # the paper's own TT benchmark (0.63 s on an A100 at lmax = 10^4): same windows, TT block alone
+        base = windows.Workload(base.name + "_tt_only", base.lmax, base.l3max, False, False, base.Wtt, None, None)
     split = bool(args.split_rows) and not base.band and base.pol and args.nwin <= 1
-    if world > 1 and not base.band and not split:
+    if world > 1 and not base.band and not split and base.pol:
         # each rank: its own window set of the same recipe (independent problems, weak scaling)
         spec = {1: ((0.7, 30.0, 2.5), (0.5, 50.0, 3.0), False), 2: ((0.6, 40.0, 2.2), (0.45, 60.0, 2.8), True),
                 3: ((0.4, 80.0, 2.0), (0.35, 100.0, 2.4), False)}.get(args.config)
