@@ -56,7 +56,7 @@ namespace {
 // 4-warp CTAs: TS = 24 148.8 ms, 48 143.4 ms, 96 141.7 ms; at lmax = 2000 96 is 1-1.6 % better than 48 as well, now
 // that the last stage is cut at the band's last block)
 constexpr int TS_DENSE = 96;      // dense polarised sweeps
-constexpr int TS_SPIN1 = 48;      // spin-1 sweeps (as measured in round 1)
+constexpr int TS_SPIN1 = 96;      // spin-1 sweeps (measured at lmax = 10^4: 48: 100.24 ms per call, 96: 99.39 ms; lmax = 2000: 0.970 / 0.957 ms)
 constexpr int TS_BAND = 64;       // band-limited sweeps (measured at config 4: 32: 0.3444 ms, 48: 0.3416, 64: 0.3417, 96: 0.3508)
 constexpr bool PIPE_DENSE = true; // TE/EE accumulations of step t issued at the start of step t+1
 constexpr int NBUF = 2;   // buffers per warp
