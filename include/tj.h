@@ -32,6 +32,7 @@ extern "C" {
                             an output requested without its window */
 #define TJ_ENOMEM  (-2)  /* host or device allocation failed */
 #define TJ_ECUDA   (-3)  /* CUDA runtime / launch error; text via tj_strerror(TJ_ECUDA) */
+#define TJ_ELIMIT  (-4)  /* tj_coupling_pol_static only: the problem needs more scratch than the built-in array holds */
 
 /* Opaque handle owning the device-resident lookup tables for one (lmax, l3max) on ONE device: the device that is
  * current when tj_build_tables is called.  Every later call with the handle must be made with the same device
@@ -81,6 +82,49 @@ int tj_coupling_pol(const tj_tables *tables,
                     const double *d_Wtt, const double *d_Wtp, const double *d_Wpp, int nW,
                     double *d_TT, double *d_TE, double *d_EE, double *d_BB, double *d_EB,
                     void *cuda_stream);
+
+/*
+ * tj_coupling_pol_static -- tj_coupling_pol for callers that must not allocate GPU memory.
+ *
+ * Who needs it.  Every other coupling call above lmax = 800 takes a little scratch (the pre-folded windows and the
+ * tile schedule, about 112 bytes per unit of lmax) from the device's stream-ordered pool with cudaMallocAsync and
+ * gives it back with cudaFreeAsync.  Some programs cannot afford that: a host application that has already
+ * claimed the whole of device memory for its own arena, so that any allocation made behind its back fails or
+ * eats into what it thought it owned; a service with a hard latency budget, where the allocator's lock and the
+ * chance that the pool has to grow (which can stall the whole device) are not acceptable inside the loop; and
+ * deployments where the stream-ordered pool is not offered at all (some virtualised and partitioned GPU set-ups).
+ * For them this entry point runs the same three kernels as tj_coupling_pol -- window pre-fold + tile schedule,
+ * staged l3 sweep, mirrored writer (PAPER.md:76-84 Eqs. 3-4, :340-356 Eqs. A1-A4) -- with the scratch in an array
+ * that is part of the library image.  It calls no cudaMalloc / cudaMallocAsync / cudaFree and no library routine
+ * that allocates; it creates no stream and no event, and records no profiling events (tj_profile_get does not
+ * see it).  The caller still owns and passes the windows and the output matrices.
+ *
+ * The limit.  The array is TJ_STATIC_SCRATCH_BYTES = 2 MiB, enough for any handle with lmax <= TJ_STATIC_LMAX =
+ * 16384 (any l3max).  Each GPU on which the library is loaded sets those 2 MiB aside until the process exits,
+ * whether or not this function is ever called.  A handle with a larger lmax is refused with TJ_ELIMIT before
+ * anything is enqueued; outputs are then untouched.
+ *
+ * Set-up.  The first call on each device looks up the device address of the array (one cudaGetSymbolAddress, made
+ * with the handle's device current, remembered per device for the life of the process).  Make that first call
+ * during start-up, before any stream capture begins.  Later calls only enqueue the three kernels.
+ *
+ * Sharing.  There is ONE array per device and every call on that device uses it.  Nothing in it has to be cleared
+ * between calls: the first kernel of a call rewrites every element the other two read (guard bands and tile
+ * schedule included), so a call never sees the previous call's contents -- but two calls that may run on the GPU
+ * at the same time (different streams, or different threads on different streams) race on it and give wrong
+ * results.  Keep all calls on one device in one stream, or order them with events.
+ *
+ * Arguments, layout, NULL rules, BB = EE and the results are exactly those of tj_coupling_pol; above lmax = 800
+ * the two agree bit for bit (same kernels, same arithmetic), at or below it tj_coupling_pol takes its single-launch
+ * path and the two agree to rounding.  Errors: TJ_EINVAL as tj_coupling_pol; TJ_ELIMIT as above; TJ_ECUDA if the
+ * address look-up or a launch fails.
+ */
+#define TJ_STATIC_LMAX           16384
+#define TJ_STATIC_SCRATCH_BYTES  (2 * 1024 * 1024)
+int tj_coupling_pol_static(const tj_tables *tables,
+                           const double *d_Wtt, const double *d_Wtp, const double *d_Wpp, int nW,
+                           double *d_TT, double *d_TE, double *d_EE, double *d_BB, double *d_EB,
+                           void *cuda_stream);
 
 /*
  * tj_coupling_band -- band-limited variant: the l3 sum stops at lcut (inclusive),

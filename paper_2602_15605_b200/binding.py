@@ -13,12 +13,13 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _SO = os.path.join(_HERE, "libtj.so")
 _LIB = None
 
-TJ_OK, TJ_EINVAL, TJ_ENOMEM, TJ_ECUDA = 0, -1, -2, -3
+TJ_OK, TJ_EINVAL, TJ_ENOMEM, TJ_ECUDA, TJ_ELIMIT = 0, -1, -2, -3, -4
+TJ_STATIC_LMAX = 16384              # include/tj.h: largest lmax tj_coupling_pol_static accepts
 
 # every symbol include/tj.h declares (tests/test_abi.py checks the header against this and the .so)
 SYMBOLS = (
     "tj_build_tables", "tj_free_tables", "tj_tables_info", "tj_tables_copy",
-    "tj_coupling_tt", "tj_coupling_pol", "tj_coupling_band", "tj_coupling_multi", "tj_coupling_spin1", "tj_coupling_rows", "tj_coupling_binned", "tj_coupling_literal", "tj_coupling_host",
+    "tj_coupling_tt", "tj_coupling_pol", "tj_coupling_pol_static", "tj_coupling_band", "tj_coupling_multi", "tj_coupling_spin1", "tj_coupling_rows", "tj_coupling_binned", "tj_coupling_literal", "tj_coupling_host",
     "tj_l3_range", "tj_sweep_counts", "tj_profile_enable", "tj_profile_get",
     "tj_profile_last_sweep", "tj_profile_launches", "tj_strerror",
 )
@@ -51,6 +52,7 @@ def load_library() -> ctypes.CDLL:
     L.tj_tables_copy.argtypes = [vp, ci, dp, ci]
     L.tj_coupling_tt.argtypes = [vp, vp, ci, vp, vp]
     L.tj_coupling_pol.argtypes = [vp, vp, vp, vp, ci, vp, vp, vp, vp, vp, vp]
+    L.tj_coupling_pol_static.argtypes = [vp, vp, vp, vp, ci, vp, vp, vp, vp, vp, vp]
     L.tj_coupling_band.argtypes = [vp, ci, vp, vp, vp, vp, vp, vp, vp, vp, vp]
     L.tj_coupling_multi.argtypes = [vp, ci, vp, vp, vp, ci, vp, vp, vp, vp, vp, vp]
     L.tj_coupling_spin1.argtypes = [vp, vp, vp, vp, ci, vp, vp, vp, vp, vp]
@@ -185,6 +187,25 @@ def coupling_pol(tables: Tables, Wtt, Wtp, Wpp, want=_BLOCKS, out=None, stream=N
     _check(load_library().tj_coupling_pol(tables.handle, _dev_ptr(Wtt, nW, "Wtt"), _dev_ptr(Wtp, nW, "Wtp"),
                                           _dev_ptr(Wpp, nW, "Wpp"), nW, *args, _stream_ptr(stream)), "tj_coupling_pol")
     return {k: out[k] for k in want}
+
+
+def coupling_pol_static(tables: Tables, Wtt, Wtp, Wpp, out: dict, stream=None):
+    """tj_coupling_pol_static: tj_coupling_pol for callers that may not allocate GPU memory (an application that owns
+    all of device memory already, a latency-bound loop, a GPU set-up without the stream-ordered pool).  The library's
+    scratch sits in a fixed 2 MiB device array instead of coming from cudaMallocAsync, so handles with
+    lmax > TJ_STATIC_LMAX are refused (TJError, code TJ_ELIMIT), and calls that overlap on one GPU race on that array:
+    keep them in one stream.  `out` is REQUIRED here -- dict name -> preallocated [(lmax+1),(lmax+1)] float64 CUDA
+    tensor for every block wanted; this wrapper creates no tensor either.  The first call on a device looks the
+    array's address up; make it before any stream capture.  Returns `out`."""
+    N = tables.lmax + 1
+    nW = tables.l3max + 1
+    if not out or any(k not in _BLOCKS for k in out):
+        raise TJError(TJ_EINVAL, "coupling_pol_static needs preallocated outputs named from %s" % (_BLOCKS,))
+    args = [_dev_ptr(out.get(k), N * N, k) for k in _BLOCKS]
+    _check(load_library().tj_coupling_pol_static(tables.handle, _dev_ptr(Wtt, nW, "Wtt"), _dev_ptr(Wtp, nW, "Wtp"),
+                                                 _dev_ptr(Wpp, nW, "Wpp"), nW, *args, _stream_ptr(stream)),
+           "tj_coupling_pol_static")
+    return out
 
 
 def coupling_band(tables: Tables, lcut: int, Wtt, Wtp, Wpp, want=_BLOCKS, out=None, stream=None):

@@ -135,6 +135,8 @@ int run_coupling_rows_to_host(const tj_tables *tables, const double *d_Wtt, cons
                               int nW, double *const d_out[5], double *const h_out[5], cudaStream_t st);
 int run_literal(const tj_tables *tables, const double *d_Wtt, const double *d_Wpp, int nW, double *d_TT, double *d_EE,
                 cudaStream_t st);
+int run_coupling_static(const tj_tables *tables, const double *d_Wtt, const double *d_Wtp, const double *d_Wpp, int nW,
+                        double *d_TT, double *d_TE, double *d_EE, double *d_BB, double *d_EB, cudaStream_t st);
 int run_binned(const tj_tables *tables, const double *d_Wtt, const double *d_Wtp, const double *d_Wpp, int nW, int nbins,
                const int *h_edges, const double *d_P, const double *d_Q, double *d_TT, double *d_TE, double *d_EE,
                double *d_BB, double *d_EB, cudaStream_t st);
@@ -167,6 +169,7 @@ const char *tj_strerror(int code)
         case TJ_EINVAL: return "invalid argument";
         case TJ_ENOMEM: return "out of memory";
         case TJ_ECUDA: return g_errbuf;
+        case TJ_ELIMIT: return "lmax exceeds TJ_STATIC_LMAX: the built-in scratch array of tj_coupling_pol_static is too small";
         default: return "unknown error code";
     }
 }
@@ -260,6 +263,14 @@ int tj_coupling_pol(const tj_tables *tables, const double *d_Wtt, const double *
     if (!tables) return TJ_EINVAL;
     if (nW != tables->T.l3max + 1) return TJ_EINVAL;
     return run_coupling(tables, -1, d_Wtt, d_Wtp, d_Wpp, nW, d_TT, d_TE, d_EE, d_BB, d_EB, (cudaStream_t)cuda_stream);
+}
+
+int tj_coupling_pol_static(const tj_tables *tables, const double *d_Wtt, const double *d_Wtp, const double *d_Wpp, int nW,
+                           double *d_TT, double *d_TE, double *d_EE, double *d_BB, double *d_EB, void *cuda_stream)
+{
+    if (!tables) return TJ_EINVAL;
+    if (nW != tables->T.l3max + 1) return TJ_EINVAL;
+    return run_coupling_static(tables, d_Wtt, d_Wtp, d_Wpp, nW, d_TT, d_TE, d_EE, d_BB, d_EB, (cudaStream_t)cuda_stream);
 }
 
 int tj_coupling_band(const tj_tables *tables, int lcut, const double *d_Wtt, const double *d_Wtp, const double *d_Wpp,
@@ -739,6 +750,91 @@ int run_binned(const tj_tables *tables, const double *d_Wtt, const double *d_Wtp
     cudaFreeAsync(scr, st);
     if (rc != TJ_OK) return rc;
     return e == cudaSuccess ? TJ_OK : cuda_fail(e, "tj_coupling_binned");
+}
+
+// ---- tj_coupling_pol_static: the dense call for callers that cannot allocate (include/tj.h) ------------------
+// The scratch of a dense one-window call (WSET prefolded window arrays + the tile prefix) lives in this array
+// instead of coming from cudaMallocAsync.  It is part of the module image: every device that loads libtj holds
+// its own 2 MiB copy until the process ends.  Host code must never hand the NAME to a kernel -- on the host it
+// stands for a shadow object, not for device memory; the device address comes from cudaGetSymbolAddress, asked once
+// per device with that device current (static_scratch_ptr below).
+static __device__ __align__(256) unsigned char g_static_scratch[TJ_STATIC_SCRATCH_BYTES];
+
+constexpr int STATIC_MAX_DEVICES = 64;
+std::mutex g_static_mu;
+unsigned char *g_static_ptr[STATIC_MAX_DEVICES];   // device address of g_static_scratch on device k (NULL: not asked yet)
+
+// Device address of the array on `dev`, which must be the current device.  First use per device: one
+// cudaGetSymbolAddress (it may load the module on that device, hence "before any stream capture" in tj.h).
+int static_scratch_ptr(int dev, unsigned char **out)
+{
+    if (dev < 0 || dev >= STATIC_MAX_DEVICES) return TJ_EINVAL;
+    std::lock_guard<std::mutex> lock(g_static_mu);
+    if (!g_static_ptr[dev]) {
+        unsigned char *ptr = nullptr;
+        cudaError_t e = cudaGetSymbolAddress((void **)&ptr, g_static_scratch);
+        if (e != cudaSuccess) return cuda_fail(e, "tj_coupling_pol_static/cudaGetSymbolAddress");
+        if (!ptr) return TJ_ECUDA;
+        g_static_ptr[dev] = ptr;
+    }
+    *out = g_static_ptr[dev];
+    return TJ_OK;
+}
+
+// Same three kernels as the general path of run_coupling (prepare, staged sweep, mirrored writer), for the dense,
+// one-window, spin-2 case only; the Call is filled here rather than by coupling_begin because that one allocates.
+// Always the general path, whatever lmax: the single-launch kernel needs no scratch, but one code path keeps the
+// contract simple (this is the variant of the scratch-using path, and its limit does not depend on a threshold).
+int run_coupling_static(const tj_tables *tables, const double *d_Wtt, const double *d_Wtp, const double *d_Wpp, int nW,
+                        double *d_TT, double *d_TE, double *d_EE, double *d_BB, double *d_EB, cudaStream_t st)
+{
+    const Tables &T = tables->T;
+    if ((d_TT && !d_Wtt) || (d_TE && !d_Wtp) || ((d_EE || d_BB || d_EB) && !d_Wpp)) return TJ_EINVAL;
+    if (!d_TT && !d_TE && !d_EE && !d_BB && !d_EB) return TJ_EINVAL;
+    if (T.lmax > TJ_STATIC_LMAX) return TJ_ELIMIT;
+    { const int rcd = check_device(tables); if (rcd != TJ_OK) return rcd; }
+    g_prof.valid = false;   // no events are recorded for this call
+
+    Call C;
+    C.T = &T;
+    C.nW = nW;
+    C.TT = d_TT; C.TE = d_TE; C.EB = d_EB;
+    C.ee = d_EE ? d_EE : d_BB;
+    C.bb_copy = (d_EE && d_BB) ? d_BB : nullptr;
+    if (!d_TE && !C.ee && !d_EB) C.mask = M_TT;
+    else if (d_TT) C.mask = M_TT | M_TE | M_EE | M_EB;
+    else C.mask = M_TE | M_EE | M_EB;
+    C.R = sweep_R(C.mask, false, 1, T.lmax, false, 2);
+    C.l3max_eff = T.l3max;
+    C.N = (long long)T.lmax + 1;
+    C.row_lo = 0;
+    C.row_hi = T.lmax + 1;
+    C.ld = C.N;
+    C.ntiles = total_tiles(T.lmax, C.l3max_eff, C.R, false, C.row_lo, C.row_hi);
+    if (C.ntiles < 0) return TJ_EINVAL;
+    C.nb = num_bands(T.lmax, C.R);
+    C.ntile_w = (int)((C.N + 31) / 32);
+
+    // layout of the array: [WSET * nl_alloc doubles: wtt, wtp, wpp, wA (pairs), wB (pairs)] [tile prefix, nb+1 ints]
+    const size_t wbytes = sizeof(double) * WSET * (size_t)T.nl_alloc;
+    const size_t tbytes = sizeof(int) * (size_t)(C.nb + 1 + 1);
+    if (wbytes + tbytes > (size_t)TJ_STATIC_SCRATCH_BYTES) return TJ_ELIMIT;   // cannot happen for lmax <= TJ_STATIC_LMAX
+    unsigned char *scr = nullptr;
+    { const int rcs = static_scratch_ptr(tables->device, &scr); if (rcs != TJ_OK) return rcs; }
+    C.wtt = (double *)scr + GUARD_LO;
+    C.wtp = C.wtt + T.nl_alloc;
+    C.wpp = C.wtp + T.nl_alloc;
+    C.wA = C.wpp - GUARD_LO + T.nl_alloc + 2 * GUARD_LO;
+    C.wB = C.wA + 2 * (size_t)T.nl_alloc;
+    C.tile_start = (int *)(scr + wbytes);
+
+    // prepare_kernel writes every element of the five window arrays (index -GUARD_LO .. nl_alloc-GUARD_LO-1, so the
+    // guard bands too) and tile_start[0..nb]: nothing of an earlier call survives into what the sweep reads
+    cudaError_t e = launch_prepare(T, d_Wtt, d_Wtp, d_Wpp, nW, C.wtt, C.wtp, C.wpp, C.wA, C.wB, C.tile_start, C.R,
+                                   C.l3max_eff, false, C.row_lo, C.row_hi, st);
+    if (e == cudaSuccess) e = coupling_sweep(C, 0, C.nb, st);
+    if (e == cudaSuccess) e = coupling_write(C, 0, C.ntile_w, st);
+    return e == cudaSuccess ? TJ_OK : cuda_fail(e, "tj_coupling_pol_static");
 }
 
 // paper-literal ablation (tj_literal.cu): prefold the windows, then one thread per pair
