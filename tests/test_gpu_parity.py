@@ -134,7 +134,9 @@ def test_flat_window_closed_form_lmax700():
 
 
 def test_cfg1_recipe_lmax300_full_all_blocks():
-    wl = windows.config(1, lmax=300)   # several CTAs per band, ragged tail (301 = 2*128 + 45)
+    """lmax <= 800: a dense one-window call takes the single-launch kernel (tj_small.cu), so this is a test of
+    small_kernel; the staged sweep gets the same treatment in tests/test_gpu_staged_sweep.py."""
+    wl = windows.config(1, lmax=300)   # 301 rows: ragged against the small kernel's rows per thread and 128-thread CTAs
     K = run_pol(wl.lmax, wl.l3max, wl.Wtt, wl.Wtp, wl.Wpp)
     ref = oracle.coupling_full(wl.lmax, wl.l3max, wl.Wtt, wl.Wtp, wl.Wpp)
     for k in BLOCKS:
@@ -319,8 +321,11 @@ def _sample_pairs(lmax, n, seed, band=None):
         l2 = rng.integers(0, lmax + 1, n)
     else:
         l2 = np.clip(l1 + rng.integers(-band, band + 1, n), 0, lmax)
-    # structured: corners, diagonal, l<2 edges, tile seams (multiples of 8/16/128), last rows/cols
-    edge = np.array([0, 1, 2, 3, 7, 8, 9, 127, 128, 129, lmax - 129, lmax - 128, lmax - 9, lmax - 8, lmax - 1, lmax])
+    # structured: corners, diagonal, l<2 edges, last rows/cols, and the seams of every geometry in use: row bands of
+    # 8 / 12 / 16 / 32 rows, writer tiles of 32, stages of 96 steps, CTA column tiles of 32 (multiples +-1)
+    edge = np.array([0, 1, 2, 3, 7, 8, 9, 11, 12, 13, 31, 32, 33, 95, 96, 97, 127, 128, 129, 959, 960, 961,
+                     lmax - 129, lmax - 128, lmax - 97, lmax - 96, lmax - 95, lmax - 13, lmax - 12, lmax - 9, lmax - 8,
+                     lmax - 1, lmax])
     edge = edge[(edge >= 0) & (edge <= lmax)]
     e1, e2 = np.meshgrid(edge, edge, indexing="ij")
     if band is not None:
