@@ -72,19 +72,55 @@ struct HostPipe {
     }
 };
 
-// optional per-kernel timing of the most recent coupling call of this thread (tj_profile_*)
+// optional per-kernel timing of the most recent coupling call of this thread (tj_profile_*).  The events are kept per
+// (thread, device): an event can only be recorded on a stream of the device it was created on, and one thread may
+// drive several GPUs (one handle per device).  Profiling never decides a call's status: if an event cannot be created
+// or recorded, the rest of that call goes unprofiled and the error is cleared from the runtime's last-error slot
+// (the launchers end with cudaGetLastError(), which must report the LAUNCH).
 std::atomic<int> g_profile{0};
-struct ProfEvents { cudaEvent_t ev[5]; bool have = false; bool valid = false; };
-thread_local ProfEvents g_prof;
+constexpr int PROF_MAX_DEVICES = 64;
+struct ProfEvents { cudaEvent_t ev[5]; bool have = false; };
+struct ProfState {
+    ProfEvents dev[PROF_MAX_DEVICES];
+    int cur = -1;          // device of the call being profiled / of the last profiled call
+    bool valid = false;    // all five events of the most recent call are recorded
+    bool broken = false;   // an event call failed during the current call
+};
+thread_local ProfState g_prof;
 
 void prof_record(int i, cudaStream_t st)
 {
     if (!g_profile.load(std::memory_order_relaxed)) return;
-    if (!g_prof.have) {
-        for (int k = 0; k < 5; ++k) cudaEventCreate(&g_prof.ev[k]);
-        g_prof.have = true;
+    if (i == 0) {   // first event of a call: pick (and if need be create) the current device's events
+        g_prof.broken = false;
+        g_prof.valid = false;
+        int d = -1;
+        if (cudaGetDevice(&d) != cudaSuccess || d < 0 || d >= PROF_MAX_DEVICES) {
+            cudaGetLastError();
+            g_prof.cur = -1;
+            return;
+        }
+        g_prof.cur = d;
+        ProfEvents &E = g_prof.dev[d];
+        if (!E.have) {
+            int made = 0;
+            while (made < 5 && cudaEventCreate(&E.ev[made]) == cudaSuccess) ++made;
+            if (made < 5) {
+                cudaGetLastError();
+                while (made > 0) cudaEventDestroy(E.ev[--made]);
+                g_prof.broken = true;
+                return;
+            }
+            E.have = true;
+        }
     }
-    cudaEventRecord(g_prof.ev[i], st);
+    if (g_prof.cur < 0 || g_prof.broken || !g_prof.dev[g_prof.cur].have) return;
+    if (cudaEventRecord(g_prof.dev[g_prof.cur].ev[i], st) != cudaSuccess) {
+        cudaGetLastError();
+        g_prof.broken = true;
+        g_prof.valid = false;
+        return;
+    }
     if (i == 4) g_prof.valid = true;
 }
 
@@ -453,12 +489,13 @@ int tj_profile_enable(int on)
 int tj_profile_get(double *h_ms3)
 {
     if (!h_ms3) return TJ_EINVAL;
-    if (!g_prof.have || !g_prof.valid) return TJ_EINVAL;
-    TJ_CUDA(cudaEventSynchronize(g_prof.ev[4]), "tj_profile_get");
+    if (g_prof.cur < 0 || !g_prof.valid || !g_prof.dev[g_prof.cur].have) return TJ_EINVAL;
+    const cudaEvent_t *ev = g_prof.dev[g_prof.cur].ev;
+    TJ_CUDA(cudaEventSynchronize(ev[4]), "tj_profile_get");
     float a = 0.f, b = 0.f, c = 0.f;
-    TJ_CUDA(cudaEventElapsedTime(&a, g_prof.ev[0], g_prof.ev[1]), "tj_profile_get");
-    TJ_CUDA(cudaEventElapsedTime(&b, g_prof.ev[2], g_prof.ev[3]), "tj_profile_get");
-    TJ_CUDA(cudaEventElapsedTime(&c, g_prof.ev[3], g_prof.ev[4]), "tj_profile_get");
+    TJ_CUDA(cudaEventElapsedTime(&a, ev[0], ev[1]), "tj_profile_get");
+    TJ_CUDA(cudaEventElapsedTime(&b, ev[2], ev[3]), "tj_profile_get");
+    TJ_CUDA(cudaEventElapsedTime(&c, ev[3], ev[4]), "tj_profile_get");
     h_ms3[0] = a; h_ms3[1] = b; h_ms3[2] = c;
     return TJ_OK;
 }

@@ -9,9 +9,10 @@
 // mirror (2 l1+1) Xi directly (steps a5-a6).  No scratch, no tile list, no second pass.
 //
 // The arithmetic per entry is, operation for operation and in the same order of l3, that of tj_sweep.cu /
-// tj_writer.cu, so results are bit-identical to the general path: the band-limited, row-block,
-// batched and host-buffer calls -- which always take the general path -- are compared bit for bit with this one in
-// tests/test_gpu_parity.py.
+// tj_writer.cu, so results are bit-identical to the general path.  tests/test_zz_no_alloc.py holds the
+// two against each other at the same sizes (tj_coupling_pol_static always runs the general path); the band-limited,
+// row-block, batched and host-buffer tests of tests/test_gpu_parity.py compare general-path variants with
+// general-path calls above LMAX_SMALL (or this kernel with itself below it), not the two with each other.
 #include "tj_internal.cuh"
 
 namespace tj {

@@ -516,7 +516,7 @@ thread_local long long g_launch_count = 0;
 
 // Geometry per request: dense sweeps are long (up to lmax steps per pair), so the per-step
 // overhead (prefactors, table reads) is spread over R = 12 pairs at 2 CTAs/SM with stages of 96 (48) steps;
-// band-limited sweeps have <= lcut/2+1 steps per pair, so they keep R = 8 and short stages of 32 steps.
+// band-limited sweeps have <= lcut/2+1 steps per pair, so they keep R = 8 and stages of TS_BAND = 64 steps (TT alone: 32).
 // Multi-window batching (nw window sets in one sweep): the geometric part of a term (r, A2, rA, rAA) is
 // computed once and each window set adds 3 FMAs (1 in the odd branch); the accumulators of nw sets take the
 // registers that R = 12 pairs use otherwise, hence R = 8 for nw = 2 and R = 6 for nw = 3.
