@@ -219,7 +219,8 @@ int tj_coupling_literal(const tj_tables *tables, const double *d_Wtt, const doub
 
 /*
  * Host-buffer forms (the end-to-end path): same semantics, but every window and output is a HOST
- * pointer (h_*; pinned memory makes the copies asynchronous and fast, pageable memory also works).
+ * pointer (h_*; pinned memory makes the copies asynchronous and fast; pageable memory also works, without the overlap
+ * of copies and arithmetic -- see tj_set_host_pipeline).
  * The call allocates device scratch from the stream-ordered pool, copies the windows in, runs the same
  * kernels, copies every requested matrix back and SYNCHRONISES the stream before returning.
  * band = 0: dense outputs, nW_or_lcut = nW = l3max+1;  band = 1: banded outputs, nW_or_lcut = lcut.
@@ -228,6 +229,28 @@ int tj_coupling_host(const tj_tables *tables, int band, int nW_or_lcut,
                      const double *h_Wtt, const double *h_Wtp, const double *h_Wpp,
                      double *h_TT, double *h_TE, double *h_EE, double *h_BB, double *h_EB,
                      void *cuda_stream);
+
+/*
+ * tj_set_host_pipeline -- what the dense host-buffer call assumes about the machine.  tj_coupling_host (band = 0, lmax
+ * above the single-launch threshold, pinned outputs) overlaps its device-to-host copies with the arithmetic, chunk of
+ * rows by chunk of rows, in one of two ways: when the copies take longer than the arithmetic, whole rows leave as soon
+ * as they are final, in many small chunks, so that the copy engine never waits ("copy-bound", regime 1); otherwise,
+ * after every chunk, the L-shaped region that chunk made final leaves as two pitched rectangles, so that almost
+ * nothing is left to copy when the last row is computed ("compute-bound", regime 2).  The choice compares
+ *     (matrices requested) * (lmax+1)^2 * 8 / d2h_bytes_per_s     with     c * (lmax+1)^3 / 6 / fp64_instr_per_s,
+ * c = 13 FP64 instructions per (even + odd) step for the polarised sweep, 2 for TT alone.  The rates are properties of
+ * the box, not of the method: the defaults, 54e9 B/s and 1.6e13 instr/s, were measured on the B200 machines the library
+ * was tuned on (PCIe Gen5 x16 to pinned memory).  On another host link -- or with several GPUs behind one
+ * PCIe switch -- pass what you measure.  0 restores a default.  Per handle; takes effect from the next call; results
+ * do not depend on it (both regimes give the same bits), only the time does.  Outputs in PAGEABLE memory are a third
+ * case (regime 3): copies into pageable memory block the calling thread, so nothing could overlap; the call then
+ * computes everything and copies each matrix out in one piece.
+ *
+ * tj_host_pipeline_info -- which regime the most recent dense host-buffer call on this handle took (0: none yet,
+ * 1, 2, 3 as above) and in how many row chunks.  Output pointers may be NULL.
+ */
+int tj_set_host_pipeline(tj_tables *tables, double d2h_bytes_per_s, double fp64_instr_per_s);
+int tj_host_pipeline_info(const tj_tables *tables, int *regime, int *nchunks);
 
 /*
  * tj_l3_range -- host-side integer bookkeeping of the l3 sum for one pair: l3 runs over

@@ -19,7 +19,7 @@ TJ_STATIC_LMAX = 16384              # include/tj.h: largest lmax tj_coupling_pol
 # every symbol include/tj.h declares (tests/test_abi.py checks the header against this and the .so)
 SYMBOLS = (
     "tj_build_tables", "tj_free_tables", "tj_tables_info", "tj_tables_copy",
-    "tj_coupling_tt", "tj_coupling_pol", "tj_coupling_pol_static", "tj_coupling_band", "tj_coupling_multi", "tj_coupling_spin1", "tj_coupling_rows", "tj_coupling_binned", "tj_coupling_literal", "tj_coupling_host",
+    "tj_coupling_tt", "tj_coupling_pol", "tj_coupling_pol_static", "tj_coupling_band", "tj_coupling_multi", "tj_coupling_spin1", "tj_coupling_rows", "tj_coupling_binned", "tj_coupling_literal", "tj_coupling_host", "tj_set_host_pipeline", "tj_host_pipeline_info",
     "tj_l3_range", "tj_sweep_counts", "tj_profile_enable", "tj_profile_get",
     "tj_profile_last_sweep", "tj_profile_launches", "tj_strerror",
 )
@@ -60,6 +60,8 @@ def load_library() -> ctypes.CDLL:
     L.tj_coupling_binned.argtypes = [vp, vp, vp, vp, ci, ci, ip, vp, vp, vp, vp, vp, vp, vp, vp]
     L.tj_coupling_literal.argtypes = [vp, vp, vp, ci, vp, vp, vp]
     L.tj_coupling_host.argtypes = [vp, ci, ci, vp, vp, vp, vp, vp, vp, vp, vp, vp]
+    L.tj_set_host_pipeline.argtypes = [vp, ctypes.c_double, ctypes.c_double]
+    L.tj_host_pipeline_info.argtypes = [vp, ip, ip]
     L.tj_l3_range.argtypes = [ci, ci, ci, ci, ip, ip, ip]
     L.tj_sweep_counts.argtypes = [ci, ci, ci, ip, ip, ip, ip]
     L.tj_profile_enable.argtypes = [ci]
@@ -327,6 +329,20 @@ def coupling_host(tables: Tables, Wtt, Wtp, Wpp, out: dict, band_lcut: int | Non
     _check(load_library().tj_coupling_host(tables.handle, band, n, _host_ptr(Wtt, nw, "Wtt"), _host_ptr(Wtp, nw, "Wtp"),
                                            _host_ptr(Wpp, nw, "Wpp"), *args, _stream_ptr(stream)), "tj_coupling_host")
     return out
+
+
+def set_host_pipeline(tables: Tables, d2h_bytes_per_s: float = 0.0, fp64_instr_per_s: float = 0.0) -> None:
+    """tj_set_host_pipeline: the machine rates behind the regime choice of the dense host-buffer call (0: default)."""
+    _check(load_library().tj_set_host_pipeline(tables.handle, float(d2h_bytes_per_s), float(fp64_instr_per_s)),
+           "tj_set_host_pipeline")
+
+
+def host_pipeline_info(tables: Tables):
+    """tj_host_pipeline_info: (regime, row chunks) of the handle's most recent dense host-buffer call;
+    regime 0 none yet, 1 copy-bound (whole rows), 2 compute-bound (L-shaped regions), 3 pageable outputs."""
+    a, b = ctypes.c_int(), ctypes.c_int()
+    _check(load_library().tj_host_pipeline_info(tables.handle, ctypes.byref(a), ctypes.byref(b)), "tj_host_pipeline_info")
+    return a.value, b.value
 
 
 def l3_range(l1, l2, l3max, parity):

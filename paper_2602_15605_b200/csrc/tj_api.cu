@@ -42,12 +42,18 @@ void tune_pool(int dev)
 // i.e. to ONE device: created on first use, destroyed by tj_free_tables; the mutex serialises host-buffer calls that
 // share a handle (each of them synchronises before it returns anyway).
 constexpr int PIPE_MAX_CHUNKS = 24;
+constexpr double HOST_COPY_RATE_DEFAULT = 54e9;     // bytes/s, contiguous device-to-host copy into pinned memory
+constexpr double HOST_INSTR_RATE_DEFAULT = 1.6e13;  // FP64 thread-instructions/s of the dense sweep
 struct HostPipe {
     std::mutex mu;
     cudaStream_t comp[2] = {nullptr, nullptr}, copy = nullptr;
     cudaEvent_t ev[PIPE_MAX_CHUNKS + 2];
     int nev = 0;
     bool have = false;
+    // what the regime choice of run_coupling_rows_to_host assumes about the machine (tj_set_host_pipeline); the
+    // defaults are the values measured on the B200 boxes this library was tuned on
+    double copy_rate = HOST_COPY_RATE_DEFAULT, instr_rate = HOST_INSTR_RATE_DEFAULT;
+    int last_regime = 0, last_chunks = 0;   // tj_host_pipeline_info
     cudaError_t ensure()
     {
         if (have) return cudaSuccess;
@@ -426,10 +432,27 @@ int tj_coupling_host(const tj_tables *tables, int band, int nW_or_lcut, const do
         int j = 0;
         for (int k = 0; k < 5; ++k)
             if (ho[k] && !(k == 3 && bb_from_ee)) dop[k] = dout + per * (size_t)(j++);
-        if (!band && !use_small_path(T, -1, 1, 2)) {
+        // The chunked pipeline needs copies that are asynchronous to the host: into pageable memory every
+        // cudaMemcpy(2D)Async blocks the issuing thread until the copy is done, so chunk k+1 would not even be enqueued
+        // before copy k has finished and the pipeline would run as compute, copy, compute, copy.  With any pageable
+        // output the call therefore computes first and then copies each matrix out in one piece.
+        bool pageable = false;
+        for (int k = 0; k < 5 && !pageable; ++k) {
+            if (!ho[k]) continue;
+            cudaPointerAttributes at;
+            if (cudaPointerGetAttributes(&at, ho[k]) != cudaSuccess) { cudaGetLastError(); pageable = true; }
+            else pageable = (at.type == cudaMemoryTypeUnregistered);
+        }
+        if (!band && !use_small_path(T, -1, 1, 2) && !pageable) {
             // dense: sweep, writer and the copies to the host pipelined by row chunks
             rc = run_coupling_rows_to_host(tables, dwp[0], dwp[1], dwp[2], nW, dop, ho, st);
         } else {
+            if (!band && !use_small_path(T, -1, 1, 2)) {
+                HostPipe &pipe = const_cast<tj_tables *>(tables)->pipe;
+                std::lock_guard<std::mutex> lock(pipe.mu);
+                pipe.last_regime = 3;
+                pipe.last_chunks = 1;
+            }
             rc = run_coupling(tables, lcut, dwp[0], dwp[1], dwp[2], nW, dop[0], dop[1], dop[2], dop[3], dop[4], st);
             if (rc == TJ_OK) {
                 for (int k = 0; k < 5 && e == cudaSuccess; ++k) {
@@ -445,6 +468,25 @@ int tj_coupling_host(const tj_tables *tables, int band, int nW_or_lcut, const do
     if (rc != TJ_OK) return rc;
     if (e != cudaSuccess) return cuda_fail(e, "tj_coupling_host/copies");
     if (es != cudaSuccess) return cuda_fail(es, "tj_coupling_host/sync");
+    return TJ_OK;
+}
+
+int tj_set_host_pipeline(tj_tables *tables, double d2h_bytes_per_s, double fp64_instr_per_s)
+{
+    if (!tables || !(d2h_bytes_per_s >= 0.0) || !(fp64_instr_per_s >= 0.0)) return TJ_EINVAL;   // NaN fails both
+    std::lock_guard<std::mutex> lock(tables->pipe.mu);
+    tables->pipe.copy_rate = d2h_bytes_per_s > 0.0 ? d2h_bytes_per_s : HOST_COPY_RATE_DEFAULT;
+    tables->pipe.instr_rate = fp64_instr_per_s > 0.0 ? fp64_instr_per_s : HOST_INSTR_RATE_DEFAULT;
+    return TJ_OK;
+}
+
+int tj_host_pipeline_info(const tj_tables *tables, int *regime, int *nchunks)
+{
+    if (!tables) return TJ_EINVAL;
+    HostPipe &pipe = const_cast<tj_tables *>(tables)->pipe;
+    std::lock_guard<std::mutex> lock(pipe.mu);
+    if (regime) *regime = pipe.last_regime;
+    if (nchunks) *nchunks = pipe.last_chunks;
     return TJ_OK;
 }
 
@@ -905,7 +947,7 @@ int run_coupling_rows_to_host(const tj_tables *tables, const double *d_Wtt, cons
     if (rc != TJ_OK) return rc;
 
     // Which regime?  Device-to-host copies reach ~54 GB/s when contiguous and ~35 GB/s as pitched rectangles (measured on
-    // this pool).  A call whose copies take longer than its arithmetic even at the contiguous rate is
+    // this pool; the rates used below are the handle's, tj_set_host_pipeline).  A call whose copies take longer than its arithmetic even at the contiguous rate is
     // COPY-BOUND (config 2: 1.0 GB = 18.5 ms against 17.3 ms of compute): there every byte must move at the contiguous
     // rate and the copy engine must never wait, so whole rows go out, chunk after chunk, in many small chunks (a row
     // is final when its own chunk is done: its left part was mirrored there by the chunks above).  Otherwise the call
@@ -914,9 +956,9 @@ int run_coupling_rows_to_host(const tj_tables *tables, const double *d_Wtt, cons
     // below), so that the last rows, cheap to compute but as long as any other, are nearly all on the host already.
     int nmat_host = 0;
     for (int m = 0; m < 5; ++m) nmat_host += h_out[m] ? 1 : 0;
-    const double copy_s = (double)nmat_host * (double)C.N * (double)C.N * 8.0 / 54e9;
+    const double copy_s = (double)nmat_host * (double)C.N * (double)C.N * 8.0 / pipe.copy_rate;
     const double n3 = (double)C.N * (double)C.N * (double)C.N / 6.0;   // even (and odd) steps of the upper triangle
-    const double comp_s = (C.mask == M_TT ? 2.0 : 13.0) * n3 / 1.6e13;
+    const double comp_s = (C.mask == M_TT ? 2.0 : 13.0) * n3 / pipe.instr_rate;
     const bool rows_mode = copy_s > comp_s;
     // chunk ends as fractions of the rows.  Compute-bound: a first chunk of 20 % of the rows is 10 % of the work and
     // releases 36 % of the bytes (measured at config 3: 4 chunks 163 ms, 6 chunks 145 ms, these 10 chunks 135.4 ms;
@@ -943,6 +985,8 @@ int run_coupling_rows_to_host(const tj_tables *tables, const double *d_Wtt, cons
         long long r = (k == nfrac - 1) ? C.N : (long long)(frac[k] * (double)C.N) / L * L;
         if (r > bound[nchunk]) bound[++nchunk] = (int)r;
     }
+    pipe.last_regime = rows_mode ? 1 : 2;
+    pipe.last_chunks = nchunk;
     cudaEvent_t *ev = pipe.ev;
     cudaEvent_t fork = ev[PIPE_MAX_CHUNKS], join = ev[PIPE_MAX_CHUNKS + 1];
     cudaError_t e = cudaEventRecord(fork, st);
