@@ -263,6 +263,12 @@ def main():
                          "exchange; strong scaling) instead of one independent window set per rank (the default, weak)")
     ap.add_argument("--ablation", action="store_true",
                     help="also time tj_coupling_literal (the paper's per-pair Eq. 10 / Eq. 16 evaluation) on the same workload")
+    ap.add_argument("--spin1", action="store_true",
+                    help="variant line: time tj_coupling_spin1 (K00, K01, K11+, K11-; 6 / 2 FP64 instructions per even / odd term)")
+    ap.add_argument("--binned", type=int, default=0, metavar="W",
+                    help="variant line: time tj_coupling_binned with bins of W multipoles from l = 2 (W >= lmax: one bin)")
+    ap.add_argument("--rows", default="", metavar="R0:R1",
+                    help="variant line: time tj_coupling_rows on the full rows R0 <= l1 < R1 (one rank's share of --split-rows)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-cpu-table-method", action="store_true")
@@ -324,7 +330,28 @@ def main():
         out = {k: torch.empty((nwin, N, width), dtype=torch.float64, device="cuda") for k in blocks}
     else:
         out = {k: torch.empty((N, width), dtype=torch.float64, device="cuda") for k in blocks}
+    # variant lines: other entry points on the same workload, one GPU, so that every number DESIGN.md quotes comes from a
+    # bench line (no e2e leg, no oracle leg: their parity lives in tests/)
+    variant = "spin1" if args.spin1 else "binned" if args.binned > 0 else "rows" if args.rows else None
+    bin_edges = bin_P = bin_Q = None
+    if variant:
+        assert wl.pol and not wl.band and nwin == 1 and world == 1 and not split, "variant lines need a dense polarised config on one GPU"
+        args.no_e2e = True
+        args.no_cpu_baseline = True
+    if variant == "spin1":
+        blocks = ("K00", "K01", "K11p", "K11m")
+        out = {k: torch.empty((N, N), dtype=torch.float64, device="cuda") for k in blocks}
+    elif variant == "binned":
+        bin_edges = list(range(2, wl.lmax + 1, args.binned)) + [wl.lmax + 1]
+        lv = np.arange(N, dtype=np.float64)
+        bin_P = torch.as_tensor(lv * (lv + 1) / (2 * np.pi) / args.binned).cuda()       # a band-power operator and its inverse
+        bin_Q = torch.as_tensor(np.where(lv > 0, 2 * np.pi / np.maximum(lv * (lv + 1), 1.0), 0.0)).cuda()
+        out = {k: torch.empty((len(bin_edges) - 1,) * 2, dtype=torch.float64, device="cuda") for k in blocks}
     row_lo, row_hi = 0, N
+    if variant == "rows":
+        row_lo, row_hi = (int(x) for x in args.rows.split(":"))
+        assert 0 <= row_lo < row_hi <= N
+        out = {k: torch.empty((row_hi - row_lo, N), dtype=torch.float64, device="cuda") for k in blocks}
     if split:
         # one problem, rank r computes the full rows of block r; the e2e leg is not defined for it
         row_lo, row_hi = shard.row_blocks(wl.lmax, world)[rank]
@@ -333,9 +360,13 @@ def main():
     flush = torch.empty(512 * 1024 * 1024 // 8, dtype=torch.float64, device="cuda")
 
     def step():
-        if split:
+        if split or variant == "rows":
             if row_hi > row_lo:
                 binding.coupling_rows(T, *dW, row_lo, row_hi, want=blocks, out=out)
+        elif variant == "spin1":
+            binding.coupling_spin1(T, *dW, want=blocks, out=out)
+        elif variant == "binned":
+            binding.coupling_binned(T, *dW, bin_edges, bin_P, bin_Q, want=blocks, out=out)
         elif nwin > 1:
             binding.coupling_multi(T, *dW, want=blocks, out=out)
         elif wl.band:
@@ -439,13 +470,19 @@ def main():
     sweep_ms = statistics.mean(k[1] for k in kern)
     prep_ms = statistics.mean(k[0] for k in kern)
     writer_ms = statistics.mean(k[2] for k in kern)
-    if split and world > 1:
+    if (split and world > 1) or variant == "rows":
         # rank 0's launch sweeps its own upper-triangle rows plus the pairs (l1 < row_lo, l2 in the block)
         nb = row_hi - row_lo
         Eb = sum((l + 1) * (N - l) for l in range(row_lo, row_hi)) + nb * (row_lo * (row_lo + 1) // 2)
         Ob = sum(l * (N - l) for l in range(row_lo, row_hi)) + nb * (row_lo * (row_lo - 1) // 2)
         alg_instr = INSTR_EVEN_POL * Eb + INSTR_ODD * Ob
         alg_flops = 12 * Eb + 6 * Ob
+        if variant == "rows":
+            terms = Eb + Ob
+            value = shard.whole_job_throughput(terms, args.steps, total_ms, 1)
+    elif variant == "spin1":
+        alg_instr = 6 * E + 2 * O          # DESIGN.md 3 item 6: K00 2 + K01 2 + K11+ 2 per even term, K11- 2 per odd term
+        alg_flops = 9 * E + 3 * O
     elif wl.pol:
         alg_instr = INSTR_EVEN_POL * E + INSTR_ODD * O
         alg_flops = 12 * E + 6 * O
@@ -467,7 +504,7 @@ def main():
         alg_instr = (5 + 3 * last) * E + (4 + last) * O
         alg_flops = (6 + 6 * last) * E + (4 + 2 * last) * O
     peaks, peak_kind = _peaks()
-    traffic, traffic_src = _traffic(wl.name if nwin == 1 and not split else None, geo)
+    traffic, traffic_src = _traffic(wl.name if nwin == 1 and not split and not variant else None, geo)
     sm_max = float(clocks.get("sm_max_mhz") or peaks.get("sm_max_mhz", 1965.0))
     peak_instr = SM_COUNT * FP64_LANES_PER_SM * sm_max * 1e6          # thread-instr/s at max boost
     achieved = alg_instr / (sweep_ms * 1e-3)
@@ -488,7 +525,8 @@ def main():
     writer_bytes = int(nmirror * 1.5 * N * width * 8 + (N * width * 8 if "BB" in blocks else 0))
     roofline = {
         # the instantiation the library really launched (tj_profile_last_sweep), not a label typed here
-        "bound": "alu", "kernel": geo["name"] + (" (last group of the call)" if nwin > 1 else ""),
+        "bound": "alu", "kernel": geo["name"] + (" (last group of the call)" if nwin > 1 else "")
+                                  + (" -- all row chunks of the call, bin kernels included in the time" if variant == "binned" else ""),
         "achieved": achieved / 1e12, "peak": peak_instr / 1e12, "unit": "T FP64 thread-instr/s",
         "frac": achieved / peak_instr,
         # dram__bytes_read.sum + dram__bytes_write.sum of one launch of this kernel, from the committed ncu --set full
@@ -507,7 +545,8 @@ def main():
                             else "library CUDA events in a separate profiled pass of the same steps after the timed region",
         "sweep_share_of_step": sweep_ms / (total_ms / args.steps) if world == 1 else None,
         # writer: per mirrored block reads the upper triangle (N^2/2) and writes N^2; BB is one more N^2 write
-        "writer": {"bound": "hbm", "achieved": writer_bytes / (writer_ms * 1e-3) / 1e9, "peak": peaks.get("hbm_gbs"),
+        "writer": None if (variant in ("rows", "binned") or split or writer_ms <= 0.0) else
+                  {"bound": "hbm", "achieved": writer_bytes / (writer_ms * 1e-3) / 1e9, "peak": peaks.get("hbm_gbs"),
                    "unit": "GB/s", "frac": writer_bytes / (writer_ms * 1e-3) / 1e9 / peaks.get("hbm_gbs"),
                    "peak_kind": peak_kind, "algorithmic_bytes": writer_bytes},
     }
@@ -572,7 +611,7 @@ def main():
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": total_ms / args.steps, "higher_is_better": True,
             "scaling": "strong" if split else "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": wl.name, "lmax": wl.lmax, "l3max": wl.l3max, "blocks": "+".join(blocks), "window_sets_per_step": nwin,
+            "config": {"workload": wl.name, "variant": variant, "bins": None if bin_edges is None else len(bin_edges) - 1, "lmax": wl.lmax, "l3max": wl.l3max, "blocks": "+".join(blocks), "window_sets_per_step": nwin,
                        "terms_even": E, "terms_odd": O, "pairs_upper": P,
                        "pairs_per_s": (1 if split else world) * P * args.steps / (total_ms * 1e-3),
                        "l2": "512 MB flush written between timed steps; each step also writes %.1f GB of output" % (bytes_out / 1e9),

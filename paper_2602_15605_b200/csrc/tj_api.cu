@@ -784,10 +784,13 @@ int run_binned(const tj_tables *tables, const double *d_Wtt, const double *d_Wtp
     if (ch > N) ch = (N + R - 1) / R * R;
     const size_t xper = (size_t)ch * (size_t)N;
     const size_t ebytes = (sizeof(int) * (size_t)(nbins + 1) + 127) & ~(size_t)127;
+    // a few wide bins: several CTAs per bin pair, their partial sums joined by a second pass (tj_binned.cu)
+    const int split = launch_bin_split(nbins);
+    const size_t pbytes = split > 1 ? (sizeof(double) * 2 * (size_t)split * (size_t)nmat * ((size_t)nbins * (nbins + 1) / 2) + 127) & ~(size_t)127 : 0;
     unsigned char *scr = nullptr;
-    TJ_CUDA(cudaMallocAsync((void **)&scr, ebytes + sizeof(double) * xper * (size_t)nmat, st), "tj_coupling_binned/scratch");
+    TJ_CUDA(cudaMallocAsync((void **)&scr, ebytes + pbytes + sizeof(double) * xper * (size_t)nmat, st), "tj_coupling_binned/scratch");
     int *d_edges = (int *)scr;
-    double *xb = (double *)(scr + ebytes);
+    double *xb = (double *)(scr + ebytes + pbytes);
     cudaError_t e = cudaMemcpyAsync(d_edges, h_edges, sizeof(int) * (size_t)(nbins + 1), cudaMemcpyHostToDevice, st);
     // the sweep's targets: one chunk buffer per requested block, in the order TT, TE, EE, EB
     double *bufs[4] = {nullptr, nullptr, nullptr, nullptr};
@@ -808,6 +811,7 @@ int run_binned(const tj_tables *tables, const double *d_Wtt, const double *d_Wtp
             e = cudaMemsetAsync(outs[m], 0, sizeof(double) * (size_t)nbins * (size_t)nbins, st);
         }
         B.edges = d_edges; B.P = d_P; B.Q = d_Q; B.nbins = nbins; B.lmax = T.lmax; B.ld = N;
+        B.split = split; B.part = split > 1 ? (double *)(scr + ebytes) : nullptr;
         prof_record(2, st);
         for (long long r0 = 0; r0 < N && e == cudaSuccess; r0 += ch) {
             const long long r1 = r0 + ch < N ? r0 + ch : N;

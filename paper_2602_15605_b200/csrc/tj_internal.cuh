@@ -157,7 +157,10 @@ struct BinParams {
     const double *P, *Q;            // device, lmax+1 weights each
     int nbins, r0, r1, lmax;
     long long ld;
+    int split;                      // CTAs per bin pair (launch_bin_split(nbins)); > 1: partial sums go through `part`
+    double *part;                   // split > 1: [nmat][nbins(nbins+1)/2][split][2] doubles of scratch
 };
+int launch_bin_split(int nbins);
 cudaError_t launch_bin(const BinParams &P, cudaStream_t st);
 
 // kernels / launchers (defined in the .cu files)

@@ -980,6 +980,42 @@ def test_binned_full_size_configs_sampled_bins(cfg, width):
     T.close()
 
 
+@pytest.mark.parametrize("lmax,edges", [(2000, [0, 2001]), (2000, [2, 300, 301, 1200, 2001]), (3000, [0, 2, 1500, 3001])])
+def test_binned_few_wide_bins_split_over_ctas(lmax, edges):
+    """One to four wide bins: each bin pair is shared by many CTAs whose partial sums a second pass adds in a fixed order
+    (tj_binned.cu).  Against the same bins formed on the host from the full matrices of tj_coupling_pol (which the tests
+    above hold against the oracle), against the oracle's own binned sums on a one-row bin, and bit-identical when repeated."""
+    import torch
+    wl = windows.config(2, lmax=lmax)
+    P, Q = _bin_weights(lmax, 3 * lmax)
+    T = binding.build_tables(lmax)
+    W = [_t(w) for w in (wl.Wtt, wl.Wtp, wl.Wpp)]
+    nb = len(edges) - 1
+    pre = {k: torch.full((nb, nb), float("nan"), dtype=torch.float64, device="cuda") for k in BLOCKS}
+    B = binding.coupling_binned(T, *W, edges, _t(P), _t(Q), out=pre)
+    again = binding.coupling_binned(T, *W, edges, _t(P), _t(Q))
+    full = binding.coupling_pol(T, *W)
+    torch.cuda.synchronize()
+    for k in BLOCKS:
+        assert torch.equal(again[k], B[k]), k
+        got = B[k].cpu().numpy()
+        K = full[k].cpu().numpy()
+        for b in range(nb):
+            for c in range(nb):
+                sl = K[edges[b]:edges[b + 1], edges[c]:edges[c + 1]]
+                want = float(P[edges[b]:edges[b + 1]] @ sl @ Q[edges[c]:edges[c + 1]])
+                scale = float(np.abs(P[edges[b]:edges[b + 1]]) @ np.abs(sl) @ np.abs(Q[edges[c]:edges[c + 1]]))
+                assert abs(got[b, c] - want) <= 1e-12 * max(scale, 1e-6), (k, b, c, got[b, c], want)
+    if nb == 4:   # the one-row bin [300, 301): its bin pairs are cheap for the oracle
+        pairs = [(1, 0), (1, 1), (1, 2), (1, 3), (0, 1), (3, 1)]
+        ref = oracle.coupling_binned(lmax, 2 * lmax, wl.Wtt, wl.Wtp, wl.Wpp, edges, P, Q, pairs=pairs)
+        for k in BLOCKS:
+            sel = ~np.isnan(ref[k])
+            assert sel.sum() == len(pairs)
+            assert_parity(B[k].cpu().numpy()[sel], ref[k][sel], "few bins %s" % k)
+    T.close()
+
+
 def test_binned_flat_window_closed_form_multi_chunk():
     """Flat window at lmax = 7000 (two chunks of rows): every bin against B = (sum_b P)(sum_b' Q (2l+1))/4 pi, TE = 0,
     EE + EB = the same on l >= 2 -- no oracle sample involved."""
