@@ -205,6 +205,23 @@ int tj_coupling_binned(const tj_tables *tables,
                        void *cuda_stream);
 
 /*
+ * tj_coupling_binned_multi -- binned output for many window sets (SURVEY.md 8(f) #1 and #4 together; PAPER.md:69-86:
+ * one coupling matrix per map pair: covariance windows): nwin window sets go through the batched
+ * sweep of tj_coupling_multi (three sets per sweep for the full set of blocks, four for TT alone; remainders as
+ * there) and each set's Xi chunks are binned as in tj_coupling_binned, so many map pairs yield nwin * nbins^2 numbers
+ * per block and never nwin full matrices.  Windows: [nwin][nW] row-major; outputs: [nwin][nbins*nbins]; bins, weights,
+ * NULL rules and BB as tj_coupling_binned.  Window set w of the result agrees with a tj_coupling_binned call on that
+ * set alone to rounding, and bit for bit while one chunk of rows holds the whole problem ((blocks) * (sets per sweep) *
+ * (lmax+1)^2 * 8 bytes <= 1 GiB): the batched sweep repeats the arithmetic per entry and the binning kernel is the
+ * same; beyond that size the two cut the rows into different chunks, whose sums are added in a different order.
+ */
+int tj_coupling_binned_multi(const tj_tables *tables, int nwin,
+                             const double *d_Wtt, const double *d_Wtp, const double *d_Wpp, int nW,
+                             int nbins, const int *h_edges, const double *d_P, const double *d_Q,
+                             double *d_TT, double *d_TE, double *d_EE, double *d_BB, double *d_EB,
+                             void *cuda_stream);
+
+/*
  * tj_coupling_literal -- ABLATION, not the hot path: the paper's own evaluation restated as
  * one plain kernel -- one thread per (l1,l2) of the upper triangle, serial l3 loop in steps of 2 with direct
  * table lookups, K^{TT} from Eq. 10 and K^{EE} from Eq. 16

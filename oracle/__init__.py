@@ -20,6 +20,7 @@ from .coupling import (  # noqa: F401
     coupling_full,
     coupling_band,
     coupling_binned,
+    coupling_binned_multi,
     spin1_pairs,
     spin1_full,
     num_threads,

@@ -222,3 +222,12 @@ def coupling_binned(lmax, l3max, Wtt, Wtp, Wpp, edges, P, Q, pairs=None):
         for k in names:
             out[k][b, c] = float(np.sum(wgt * K[k]))
     return out
+
+
+def coupling_binned_multi(lmax, l3max, Wtt, Wtp, Wpp, edges, P, Q, pairs=None):
+    """coupling_binned for several window sets (windows [nwin, l3max+1] or None): one independent problem per set
+    (one coupling matrix per map pair).  Returns dict name -> float64[nwin, nbins, nbins]."""
+    first = next(w for w in (Wtt, Wtp, Wpp) if w is not None)
+    res = [coupling_binned(lmax, l3max, None if Wtt is None else Wtt[w], None if Wtp is None else Wtp[w],
+                           None if Wpp is None else Wpp[w], edges, P, Q, pairs=pairs) for w in range(len(first))]
+    return {k: np.stack([r[k] for r in res]) for k in res[0]}

@@ -19,7 +19,7 @@ TJ_STATIC_LMAX = 16384              # include/tj.h: largest lmax tj_coupling_pol
 # every symbol include/tj.h declares (tests/test_abi.py checks the header against this and the .so)
 SYMBOLS = (
     "tj_build_tables", "tj_free_tables", "tj_tables_info", "tj_tables_copy",
-    "tj_coupling_tt", "tj_coupling_pol", "tj_coupling_pol_static", "tj_coupling_band", "tj_coupling_multi", "tj_coupling_spin1", "tj_coupling_rows", "tj_coupling_binned", "tj_coupling_literal", "tj_coupling_host", "tj_set_host_pipeline", "tj_host_pipeline_info",
+    "tj_coupling_tt", "tj_coupling_pol", "tj_coupling_pol_static", "tj_coupling_band", "tj_coupling_multi", "tj_coupling_spin1", "tj_coupling_rows", "tj_coupling_binned", "tj_coupling_binned_multi", "tj_coupling_literal", "tj_coupling_host", "tj_set_host_pipeline", "tj_host_pipeline_info",
     "tj_l3_range", "tj_sweep_counts", "tj_profile_enable", "tj_profile_get",
     "tj_profile_last_sweep", "tj_profile_launches", "tj_strerror",
 )
@@ -58,6 +58,7 @@ def load_library() -> ctypes.CDLL:
     L.tj_coupling_spin1.argtypes = [vp, vp, vp, vp, ci, vp, vp, vp, vp, vp]
     L.tj_coupling_rows.argtypes = [vp, vp, vp, vp, ci, ci, ci, vp, vp, vp, vp, vp, vp]
     L.tj_coupling_binned.argtypes = [vp, vp, vp, vp, ci, ci, ip, vp, vp, vp, vp, vp, vp, vp, vp]
+    L.tj_coupling_binned_multi.argtypes = [vp, ci, vp, vp, vp, ci, ci, ip, vp, vp, vp, vp, vp, vp, vp, vp]
     L.tj_coupling_literal.argtypes = [vp, vp, vp, ci, vp, vp, vp]
     L.tj_coupling_host.argtypes = [vp, ci, ci, vp, vp, vp, vp, vp, vp, vp, vp, vp]
     L.tj_set_host_pipeline.argtypes = [vp, ctypes.c_double, ctypes.c_double]
@@ -301,6 +302,28 @@ def coupling_binned(tables: Tables, Wtt, Wtp, Wpp, edges, P, Q, want=_BLOCKS, ou
     _check(load_library().tj_coupling_binned(tables.handle, _dev_ptr(Wtt, nW, "Wtt"), _dev_ptr(Wtp, nW, "Wtp"),
                                              _dev_ptr(Wpp, nW, "Wpp"), nW, nb, harr, _dev_ptr(P, N, "P"), _dev_ptr(Q, N, "Q"),
                                              *args, _stream_ptr(stream)), "tj_coupling_binned")
+    return {k: out[k] for k in want}
+
+
+def coupling_binned_multi(tables: Tables, Wtt, Wtp, Wpp, edges, P, Q, want=_BLOCKS, out=None, stream=None):
+    """tj_coupling_binned_multi.  Windows: float64 CUDA tensors [nwin, l3max+1]; returns dict name -> [nwin, nbins, nbins]."""
+    import torch
+    N = tables.lmax + 1
+    nW = tables.l3max + 1
+    first = next(w for w in (Wtt, Wtp, Wpp) if w is not None)
+    nwin = int(first.shape[0])
+    edges = [int(x) for x in edges]
+    nb = len(edges) - 1
+    harr = (ctypes.c_int * (nb + 1))(*edges)
+    out = {} if out is None else dict(out)
+    for k in want:
+        if k not in out:
+            out[k] = torch.empty((nwin, nb, nb), dtype=torch.float64, device=first.device)
+    args = [_dev_ptr(out.get(k) if k in want else None, nwin * nb * nb, k) for k in _BLOCKS]
+    _check(load_library().tj_coupling_binned_multi(tables.handle, nwin, _dev_ptr(Wtt, nwin * nW, "Wtt"),
+                                                   _dev_ptr(Wtp, nwin * nW, "Wtp"), _dev_ptr(Wpp, nwin * nW, "Wpp"), nW,
+                                                   nb, harr, _dev_ptr(P, N, "P"), _dev_ptr(Q, N, "Q"), *args,
+                                                   _stream_ptr(stream)), "tj_coupling_binned_multi")
     return {k: out[k] for k in want}
 
 

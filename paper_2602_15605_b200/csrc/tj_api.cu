@@ -158,6 +158,7 @@ struct Call {
     double *xit[4] = {nullptr, nullptr, nullptr, nullptr};
     long long ldT = 0;
     int dmax = 0;
+    long long ostride = 0;          // doubles between the outputs of consecutive window sets (0: whole matrices, N * ld)
 };
 
 // Dense single-window spin-2 calls at small lmax take the single-launch path (tj_small.cu): below LMAX_SMALL the
@@ -181,7 +182,7 @@ int run_coupling_static(const tj_tables *tables, const double *d_Wtt, const doub
                         double *d_TT, double *d_TE, double *d_EE, double *d_BB, double *d_EB, cudaStream_t st);
 int run_binned(const tj_tables *tables, const double *d_Wtt, const double *d_Wtp, const double *d_Wpp, int nW, int nbins,
                const int *h_edges, const double *d_P, const double *d_Q, double *d_TT, double *d_TE, double *d_EE,
-               double *d_BB, double *d_EB, cudaStream_t st);
+               double *d_BB, double *d_EB, cudaStream_t st, int nw = 1);
 
 }  // namespace
 
@@ -382,6 +383,37 @@ int tj_coupling_binned(const tj_tables *tables, const double *d_Wtt, const doubl
         if (h_edges[b + 1] < h_edges[b]) return TJ_EINVAL;
     return run_binned(tables, d_Wtt, d_Wtp, d_Wpp, nW, nbins, h_edges, d_P, d_Q, d_TT, d_TE, d_EE, d_BB, d_EB,
                       (cudaStream_t)cuda_stream);
+}
+
+int tj_coupling_binned_multi(const tj_tables *tables, int nwin, const double *d_Wtt, const double *d_Wtp,
+                             const double *d_Wpp, int nW, int nbins, const int *h_edges, const double *d_P,
+                             const double *d_Q, double *d_TT, double *d_TE, double *d_EE, double *d_BB, double *d_EB,
+                             void *cuda_stream)
+{
+    if (!tables || nwin < 1 || !h_edges || !d_P || !d_Q || nbins < 1 || nbins > 46340) return TJ_EINVAL;
+    if (nW != tables->T.l3max + 1) return TJ_EINVAL;
+    if (h_edges[0] < 0 || h_edges[nbins] > tables->T.lmax + 1) return TJ_EINVAL;
+    for (int b = 0; b < nbins; ++b)
+        if (h_edges[b + 1] < h_edges[b]) return TJ_EINVAL;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t nb2 = (size_t)nbins * (size_t)nbins;
+    // grouping as tj_coupling_multi: the batched sweeps exist for the full set of blocks (3 or 2 window sets) and for TT
+    // alone (4 or 2); any other request is binned one window set at a time
+    const bool full = d_Wtt && d_Wtp && d_Wpp && d_TT && d_TE && (d_EE || d_BB) && d_EB;
+    const bool tt_only = d_Wtt && d_TT && !d_TE && !d_EE && !d_BB && !d_EB;
+    int w = 0;
+    while (w < nwin) {
+        const int left = nwin - w;
+        const int nw = tt_only ? (left >= 4 ? 4 : left >= 2 ? 2 : 1)
+                               : !full ? 1 : (left == 4 || left == 2) ? 2 : left >= 3 ? 3 : 1;
+        const size_t wi = (size_t)w * (size_t)nW, oi = (size_t)w * nb2;
+        int rc = run_binned(tables, d_Wtt ? d_Wtt + wi : nullptr, d_Wtp ? d_Wtp + wi : nullptr, d_Wpp ? d_Wpp + wi : nullptr,
+                            nW, nbins, h_edges, d_P, d_Q, d_TT ? d_TT + oi : nullptr, d_TE ? d_TE + oi : nullptr,
+                            d_EE ? d_EE + oi : nullptr, d_BB ? d_BB + oi : nullptr, d_EB ? d_EB + oi : nullptr, st, nw);
+        if (rc != TJ_OK) return rc;
+        w += nw;
+    }
+    return TJ_OK;
 }
 
 int tj_coupling_literal(const tj_tables *tables, const double *d_Wtt, const double *d_Wpp, int nW, double *d_TT,
@@ -671,7 +703,7 @@ cudaError_t coupling_sweep(const Call &C, int b0, int b1, cudaStream_t st)
     P.tile_off = all ? 0 : tiles_above(C, b1 - 1);
     P.wstride = WSET * (long long)T.nl_alloc;
     P.row_lo = C.row_lo; P.row_hi = C.row_hi; P.rows = C.rows ? 1 : 0;
-    P.ostride = C.N * C.ld;
+    P.ostride = C.ostride ? C.ostride : C.N * C.ld;
     const int n = all ? C.ntiles : tiles_above(C, b0 - 1) - P.tile_off;
     return launch_sweep(P, C.mask, C.nw, C.mask == M_TT ? 2 : C.spin, n, st);
 }
@@ -765,9 +797,11 @@ int run_rows(const tj_tables *tables, const double *d_Wtt, const double *d_Wtp, 
 }
 
 // binned output (tj_binned.cu): the sweep runs over chunks of rows into Xi scratch, bin_kernel adds each chunk to the bins
+// nw > 1 (tj_coupling_binned_multi): windows [nw][nW], outputs [nw][nbins^2]; the batched sweep leaves the nw Xi chunks
+// of a block one after the other in its chunk buffer and every window set is binned from its own
 int run_binned(const tj_tables *tables, const double *d_Wtt, const double *d_Wtp, const double *d_Wpp, int nW, int nbins,
                const int *h_edges, const double *d_P, const double *d_Q, double *d_TT, double *d_TE, double *d_EE,
-               double *d_BB, double *d_EB, cudaStream_t st)
+               double *d_BB, double *d_EB, cudaStream_t st, int nw)
 {
     const Tables &T = tables->T;
     const long long N = (long long)T.lmax + 1;
@@ -778,8 +812,8 @@ int run_binned(const tj_tables *tables, const double *d_Wtt, const double *d_Wtp
     if ((d_TT && !d_Wtt) || (d_TE && !d_Wtp) || ((d_EE || d_BB || d_EB) && !d_Wpp)) return TJ_EINVAL;
     // rows per chunk: whole row bands of the sweep, at most ~1 GiB of Xi scratch
     const int mask = (!d_TE && !outs[2] && !d_EB) ? M_TT : (d_TT ? M_TT : 0) | M_TE | M_EE | M_EB;
-    const int R = sweep_R(mask, false, 1, T.lmax, false, 2);
-    long long ch = ((1LL << 30) / (8 * N * nmat)) / R * R;
+    const int R = sweep_R(mask, false, nw, T.lmax, false, 2);
+    long long ch = ((1LL << 30) / (8 * N * nmat * nw)) / R * R;
     if (ch < R) ch = R;
     if (ch > N) ch = (N + R - 1) / R * R;
     const size_t xper = (size_t)ch * (size_t)N;
@@ -788,7 +822,7 @@ int run_binned(const tj_tables *tables, const double *d_Wtt, const double *d_Wtp
     const int split = launch_bin_split(nbins);
     const size_t pbytes = split > 1 ? (sizeof(double) * 2 * (size_t)split * (size_t)nmat * ((size_t)nbins * (nbins + 1) / 2) + 127) & ~(size_t)127 : 0;
     unsigned char *scr = nullptr;
-    TJ_CUDA(cudaMallocAsync((void **)&scr, ebytes + pbytes + sizeof(double) * xper * (size_t)nmat, st), "tj_coupling_binned/scratch");
+    TJ_CUDA(cudaMallocAsync((void **)&scr, ebytes + pbytes + sizeof(double) * xper * (size_t)nmat * (size_t)nw, st), "tj_coupling_binned/scratch");
     int *d_edges = (int *)scr;
     double *xb = (double *)(scr + ebytes + pbytes);
     cudaError_t e = cudaMemcpyAsync(d_edges, h_edges, sizeof(int) * (size_t)(nbins + 1), cudaMemcpyHostToDevice, st);
@@ -797,18 +831,21 @@ int run_binned(const tj_tables *tables, const double *d_Wtt, const double *d_Wtp
     {
         int k = 0;
         for (int m = 0; m < 4; ++m)
-            if (outs[m]) bufs[m] = xb + xper * (size_t)(k++);
+            if (outs[m]) bufs[m] = xb + xper * (size_t)nw * (size_t)(k++);
     }
+    const size_t nb2 = (size_t)nbins * (size_t)nbins;
     Call C;
     int rc = TJ_OK;
-    if (e == cudaSuccess) rc = coupling_begin(C, tables, -1, d_Wtt, d_Wtp, d_Wpp, nW, bufs[0], bufs[1], bufs[2], nullptr, bufs[3], st);
+    if (e == cudaSuccess) rc = coupling_begin(C, tables, -1, d_Wtt, d_Wtp, d_Wpp, nW, bufs[0], bufs[1], bufs[2], nullptr, bufs[3], st, nw);
     if (e == cudaSuccess && rc == TJ_OK) {
+        C.ostride = (long long)xper;   // window set w of a block: its chunk buffer + w * xper
         BinParams B;
         memset(&B, 0, sizeof(B));
+        double *bout[4] = {nullptr, nullptr, nullptr, nullptr};
         for (int m = 0; m < 4 && e == cudaSuccess; ++m) {
             if (!outs[m]) continue;
-            B.B[B.nmat++] = outs[m];
-            e = cudaMemsetAsync(outs[m], 0, sizeof(double) * (size_t)nbins * (size_t)nbins, st);
+            bout[B.nmat++] = outs[m];
+            e = cudaMemsetAsync(outs[m], 0, sizeof(double) * nb2 * (size_t)nw, st);
         }
         B.edges = d_edges; B.P = d_P; B.Q = d_Q; B.nbins = nbins; B.lmax = T.lmax; B.ld = N;
         B.split = split; B.part = split > 1 ? (double *)(scr + ebytes) : nullptr;
@@ -816,17 +853,21 @@ int run_binned(const tj_tables *tables, const double *d_Wtt, const double *d_Wtp
         for (long long r0 = 0; r0 < N && e == cudaSuccess; r0 += ch) {
             const long long r1 = r0 + ch < N ? r0 + ch : N;
             // the sweep addresses Xi(l1,l2) as base[l1*N + l2]: shift the bases so that row r0 is row 0 of the chunk
-            int k = 0;
             double **tgt[4] = {&C.TT, &C.TE, &C.ee, &C.EB};
             for (int m = 0; m < 4; ++m)
-                if (outs[m]) { *tgt[m] = bufs[m] - r0 * N; B.X[k++] = bufs[m]; }
+                if (outs[m]) *tgt[m] = bufs[m] - r0 * N;
             e = coupling_sweep(C, (int)(r0 / C.R), r1 == N ? C.nb : (int)(r1 / C.R), st);
             B.r0 = (int)r0; B.r1 = (int)r1;
-            if (e == cudaSuccess) e = launch_bin(B, st);
+            for (int w = 0; w < nw && e == cudaSuccess; ++w) {
+                int k = 0;
+                for (int m = 0; m < 4; ++m)
+                    if (outs[m]) { B.X[k] = bufs[m] + (size_t)w * xper; B.B[k] = bout[k] + (size_t)w * nb2; ++k; }
+                e = launch_bin(B, st);
+            }
         }
         prof_record(3, st);
         if (e == cudaSuccess && d_EE && d_BB)
-            e = cudaMemcpyAsync(d_BB, d_EE, sizeof(double) * (size_t)nbins * (size_t)nbins, cudaMemcpyDeviceToDevice, st);
+            e = cudaMemcpyAsync(d_BB, d_EE, sizeof(double) * nb2 * (size_t)nw, cudaMemcpyDeviceToDevice, st);
         prof_record(4, st);
         coupling_end(C, st);
     }

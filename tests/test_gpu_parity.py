@@ -1016,6 +1016,45 @@ def test_binned_few_wide_bins_split_over_ctas(lmax, edges):
     T.close()
 
 
+@pytest.mark.parametrize("lmax,nwin,edges", [(150, 5, [0, 2, 9, 9, 40, 100, 151]), (2000, 3, list(range(2, 2001, 40)) + [2001])])
+def test_binned_multi_window_against_oracle_and_single_calls(lmax, nwin, edges):
+    """tj_coupling_binned_multi (many map pairs -> nwin * nbins^2 numbers per block, SURVEY.md 8(f) #1 + #4): against the
+    oracle (all bins at the small size, sampled bins at config-1 size) and bit for bit against nwin single-set
+    tj_coupling_binned calls (one chunk of rows at these sizes); groups of 3 + 2 sets, TT alone in 4 + 1, a partial
+    request one set at a time."""
+    import torch
+    Wtt, Wtp, Wpp = _window_sets(lmax, nwin, 40)
+    P, Q = _bin_weights(lmax, 11 * lmax)
+    T = binding.build_tables(lmax)
+    W = [_t(Wtt), _t(Wtp), _t(Wpp)]
+    nb = len(edges) - 1
+    pre = {k: torch.full((nwin, nb, nb), float("nan"), dtype=torch.float64, device="cuda") for k in BLOCKS}
+    B = binding.coupling_binned_multi(T, *W, edges, _t(P), _t(Q), out=pre)
+    geo = binding.profile_last_sweep()
+    assert geo["nw"] == (2 if nwin == 5 else 3), geo
+    torch.cuda.synchronize()
+    for w in range(nwin):
+        one = binding.coupling_binned(T, W[0][w].contiguous(), W[1][w].contiguous(), W[2][w].contiguous(), edges, _t(P), _t(Q))
+        for k in BLOCKS:
+            assert torch.equal(B[k][w], one[k]), (w, k)
+    pairs = None if lmax <= 300 else [(0, 0), (3, 11), (11, 3), (nb - 1, nb - 1), (7, 8), (nb - 1, 0)]
+    ref = oracle.coupling_binned_multi(lmax, 2 * lmax, Wtt, Wtp, Wpp, edges, P, Q, pairs=pairs)
+    for k in BLOCKS:
+        got = B[k].cpu().numpy()
+        assert np.all(np.isfinite(got)), k
+        sel = ~np.isnan(ref[k])
+        assert_parity(got[sel], ref[k][sel], "binned multi %s" % k)
+    assert torch.equal(B["BB"], B["EE"])
+    tt = binding.coupling_binned_multi(T, W[0], None, None, edges, _t(P), _t(Q), want=("TT",))
+    assert binding.profile_last_sweep()["nw"] == 1      # 4 + 1, or 2 + 1: the last sweep holds the odd set
+    pol = binding.coupling_binned_multi(T, None, W[1], W[2], edges, _t(P), _t(Q), want=("TE", "BB", "EB"))
+    torch.cuda.synchronize()
+    assert_parity(tt["TT"].cpu().numpy(), B["TT"].cpu().numpy(), "binned multi TT alone")
+    for k in ("TE", "BB", "EB"):
+        assert_parity(pol[k].cpu().numpy(), B[k].cpu().numpy(), "binned multi pol %s" % k)
+    T.close()
+
+
 def test_binned_flat_window_closed_form_multi_chunk():
     """Flat window at lmax = 7000 (two chunks of rows): every bin against B = (sum_b P)(sum_b' Q (2l+1))/4 pi, TE = 0,
     EE + EB = the same on l >= 2 -- no oracle sample involved."""
