@@ -248,6 +248,43 @@ int tj_coupling_host(const tj_tables *tables, int band, int nW_or_lcut,
                      void *cuda_stream);
 
 /*
+ * One matrix set on several GPUs, every pair swept once (each element is
+ * independent).  The rows are cut into chunks of a multiple of lcm(R, 32) rows.  What a chunk [r0, r1) makes final all
+ * by itself -- its own sweep and mirrored writer, nothing from any other chunk -- is an L-shaped region of every matrix:
+ * its rows from column r0 on, and columns [r0, r1) of all rows below.  These regions tile the matrix, so chunks can be
+ * dealt to devices: a device sweeps only the upper-triangle pairs of its own chunks and delivers exactly their
+ * regions into the ONE host matrix, over its own host link.  No pair is swept twice (tj_coupling_rows, the other way
+ * to share a matrix, sweeps every pair left of a block a second time), nothing is exchanged between devices.
+ *
+ * tj_chunk_plan -- HOST-side: the chunks and their owners for nparts devices.  Chunks are dealt by work (sweep steps,
+ * sum over a chunk's rows l1 of (l1+1)(lmax+1-l1)): heaviest first, each to the device with the least work so far.
+ * h_bounds receives nchunks+1 ascending row bounds (first 0, last lmax+1), h_owner nchunks device indices; both must
+ * have room for 12*nparts+1 entries.  tt_only selects the row-band geometry of the TT-alone sweep.  1 <= nparts <= 64.
+ *
+ * tj_coupling_host_part -- one device's share: computes the chunks tj_chunk_plan gives to `part` and writes their
+ * regions into the host matrices, leaving every other entry of h_* untouched; after the calls for part = 0..nparts-1
+ * (on any devices, in any order, also one after the other on a single GPU) the matrices are complete and carry the
+ * bits of tj_coupling_host.  Per rank under a launcher: part = rank, nparts = world size, each rank with a handle on
+ * its own device (if the ranks do not share host memory, each holds its regions and the rest of its buffer is
+ * whatever it was).  Dense outputs only; arguments as tj_coupling_host (nW = l3max+1; pinned buffers, or the copies
+ * do not overlap the arithmetic); synchronises the stream before it returns.  The single-launch path is not used here.
+ *
+ * tj_coupling_host_multi -- one process, ndev devices: tables[g] is a handle built on device g's GPU (all for the same
+ * lmax and l3max; distinct handles, which may even live on one GPU), cuda_streams[g] a stream of that device (or
+ * cuda_streams = NULL for the default streams).  Enqueues every device's share, then waits for all of them; restores
+ * the caller's current device.  h_* must be pinned for the shares to run concurrently.
+ */
+int tj_chunk_plan(int lmax, int tt_only, int nparts, int *h_bounds, int *h_owner, int *nchunks);
+int tj_coupling_host_part(const tj_tables *tables, int part, int nparts, int nW,
+                          const double *h_Wtt, const double *h_Wtp, const double *h_Wpp,
+                          double *h_TT, double *h_TE, double *h_EE, double *h_BB, double *h_EB,
+                          void *cuda_stream);
+int tj_coupling_host_multi(tj_tables *const *tables, int ndev, int nW,
+                           const double *h_Wtt, const double *h_Wtp, const double *h_Wpp,
+                           double *h_TT, double *h_TE, double *h_EE, double *h_BB, double *h_EB,
+                           void *const *cuda_streams);
+
+/*
  * tj_set_host_pipeline -- what the dense host-buffer call assumes about the machine.  tj_coupling_host (band = 0, lmax
  * above the single-launch threshold, pinned outputs) overlaps its device-to-host copies with the arithmetic, chunk of
  * rows by chunk of rows, in one of two ways: when the copies take longer than the arithmetic, whole rows leave as soon
@@ -264,7 +301,7 @@ int tj_coupling_host(const tj_tables *tables, int band, int nW_or_lcut,
  * computes everything and copies each matrix out in one piece.
  *
  * tj_host_pipeline_info -- which regime the most recent dense host-buffer call on this handle took (0: none yet,
- * 1, 2, 3 as above) and in how many row chunks.  Output pointers may be NULL.
+ * 1, 2, 3 as above, 4: one part of several, tj_coupling_host_part / _multi) and in how many row chunks.  Output pointers may be NULL.
  */
 int tj_set_host_pipeline(tj_tables *tables, double d2h_bytes_per_s, double fp64_instr_per_s);
 int tj_host_pipeline_info(const tj_tables *tables, int *regime, int *nchunks);

@@ -20,6 +20,7 @@ TJ_STATIC_LMAX = 16384              # include/tj.h: largest lmax tj_coupling_pol
 SYMBOLS = (
     "tj_build_tables", "tj_free_tables", "tj_tables_info", "tj_tables_copy",
     "tj_coupling_tt", "tj_coupling_pol", "tj_coupling_pol_static", "tj_coupling_band", "tj_coupling_multi", "tj_coupling_spin1", "tj_coupling_rows", "tj_coupling_binned", "tj_coupling_binned_multi", "tj_coupling_literal", "tj_coupling_host", "tj_set_host_pipeline", "tj_host_pipeline_info",
+    "tj_chunk_plan", "tj_coupling_host_part", "tj_coupling_host_multi",
     "tj_l3_range", "tj_sweep_counts", "tj_profile_enable", "tj_profile_get",
     "tj_profile_last_sweep", "tj_profile_launches", "tj_strerror",
 )
@@ -61,6 +62,9 @@ def load_library() -> ctypes.CDLL:
     L.tj_coupling_binned_multi.argtypes = [vp, ci, vp, vp, vp, ci, ci, ip, vp, vp, vp, vp, vp, vp, vp, vp]
     L.tj_coupling_literal.argtypes = [vp, vp, vp, ci, vp, vp, vp]
     L.tj_coupling_host.argtypes = [vp, ci, ci, vp, vp, vp, vp, vp, vp, vp, vp, vp]
+    L.tj_chunk_plan.argtypes = [ci, ci, ci, ip, ip, ip]
+    L.tj_coupling_host_part.argtypes = [vp, ci, ci, ci, vp, vp, vp, vp, vp, vp, vp, vp, vp]
+    L.tj_coupling_host_multi.argtypes = [ctypes.POINTER(vp), ci, ci, vp, vp, vp, vp, vp, vp, vp, vp, ctypes.POINTER(vp)]
     L.tj_set_host_pipeline.argtypes = [vp, ctypes.c_double, ctypes.c_double]
     L.tj_host_pipeline_info.argtypes = [vp, ip, ip]
     L.tj_l3_range.argtypes = [ci, ci, ci, ci, ip, ip, ip]
@@ -351,6 +355,42 @@ def coupling_host(tables: Tables, Wtt, Wtp, Wpp, out: dict, band_lcut: int | Non
     args = [_host_ptr(out.get(k), per, k) for k in _BLOCKS]
     _check(load_library().tj_coupling_host(tables.handle, band, n, _host_ptr(Wtt, nw, "Wtt"), _host_ptr(Wtp, nw, "Wtp"),
                                            _host_ptr(Wpp, nw, "Wpp"), *args, _stream_ptr(stream)), "tj_coupling_host")
+    return out
+
+
+def chunk_plan(lmax: int, nparts: int, tt_only: bool = False):
+    """tj_chunk_plan (host side, no GPU): (bounds, owner) -- the row chunks of a matrix shared by nparts devices and
+    the device each belongs to."""
+    cap = 12 * int(nparts) + 1
+    b, o, n = (ctypes.c_int * cap)(), (ctypes.c_int * cap)(), ctypes.c_int()
+    _check(load_library().tj_chunk_plan(int(lmax), 1 if tt_only else 0, int(nparts), b, o, ctypes.byref(n)), "tj_chunk_plan")
+    return [int(b[k]) for k in range(n.value + 1)], [int(o[k]) for k in range(n.value)]
+
+
+def coupling_host_part(tables: Tables, part: int, nparts: int, Wtt, Wtp, Wpp, out: dict, stream=None):
+    """tj_coupling_host_part: this part's share of a dense host-buffer call (HOST tensors; only the regions of the
+    part's chunks are written into `out`).  Synchronises before returning."""
+    N = tables.lmax + 1
+    nW = tables.l3max + 1
+    args = [_host_ptr(out.get(k), N * N, k) for k in _BLOCKS]
+    _check(load_library().tj_coupling_host_part(tables.handle, int(part), int(nparts), nW, _host_ptr(Wtt, nW, "Wtt"),
+                                                _host_ptr(Wtp, nW, "Wtp"), _host_ptr(Wpp, nW, "Wpp"), *args,
+                                                _stream_ptr(stream)), "tj_coupling_host_part")
+    return out
+
+
+def coupling_host_multi(tables_list, Wtt, Wtp, Wpp, out: dict, streams=None):
+    """tj_coupling_host_multi: one matrix set computed by len(tables_list) handles (one per GPU; distinct handles on
+    one GPU also work), every pair swept once, all regions delivered into the one set of HOST tensors `out`."""
+    T0 = tables_list[0]
+    N = T0.lmax + 1
+    nW = T0.l3max + 1
+    n = len(tables_list)
+    harr = (ctypes.c_void_p * n)(*[t.handle for t in tables_list])
+    sarr = None if streams is None else (ctypes.c_void_p * n)(*[s.cuda_stream for s in streams])
+    args = [_host_ptr(out.get(k), N * N, k) for k in _BLOCKS]
+    _check(load_library().tj_coupling_host_multi(harr, n, nW, _host_ptr(Wtt, nW, "Wtt"), _host_ptr(Wtp, nW, "Wtp"),
+                                                 _host_ptr(Wpp, nW, "Wpp"), *args, sarr), "tj_coupling_host_multi")
     return out
 
 

@@ -42,6 +42,7 @@ void tune_pool(int dev)
 // i.e. to ONE device: created on first use, destroyed by tj_free_tables; the mutex serialises host-buffer calls that
 // share a handle (each of them synchronises before it returns anyway).
 constexpr int PIPE_MAX_CHUNKS = 24;
+constexpr int PLAN_MAX_PARTS = 64;                  // devices that may share one matrix (tj_coupling_host_multi)
 constexpr double HOST_COPY_RATE_DEFAULT = 54e9;     // bytes/s, contiguous device-to-host copy into pinned memory
 constexpr double HOST_INSTR_RATE_DEFAULT = 1.6e13;  // FP64 thread-instructions/s of the dense sweep
 struct HostPipe {
@@ -175,7 +176,9 @@ int run_coupling(const tj_tables *tables, int lcut, const double *d_Wtt, const d
 int run_rows(const tj_tables *tables, const double *d_Wtt, const double *d_Wtp, const double *d_Wpp, int nW, int row_lo,
              int row_hi, double *d_TT, double *d_TE, double *d_EE, double *d_BB, double *d_EB, cudaStream_t st);
 int run_coupling_rows_to_host(const tj_tables *tables, const double *d_Wtt, const double *d_Wtp, const double *d_Wpp,
-                              int nW, double *const d_out[5], double *const h_out[5], cudaStream_t st);
+                              int nW, double *const d_out[5], double *const h_out[5], cudaStream_t st, int part = 0,
+                              int nparts = 1);
+int chunk_plan(int lmax, int R, int nparts, int *bounds, int *owner);
 int run_literal(const tj_tables *tables, const double *d_Wtt, const double *d_Wpp, int nW, double *d_TT, double *d_EE,
                 cudaStream_t st);
 int run_coupling_static(const tj_tables *tables, const double *d_Wtt, const double *d_Wtp, const double *d_Wpp, int nW,
@@ -501,6 +504,117 @@ int tj_coupling_host(const tj_tables *tables, int band, int nW_or_lcut, const do
     if (e != cudaSuccess) return cuda_fail(e, "tj_coupling_host/copies");
     if (es != cudaSuccess) return cuda_fail(es, "tj_coupling_host/sync");
     return TJ_OK;
+}
+
+int tj_chunk_plan(int lmax, int tt_only, int nparts, int *h_bounds, int *h_owner, int *nchunks)
+{
+    if (lmax < 0 || nparts < 1 || nparts > PLAN_MAX_PARTS || !h_bounds || !h_owner || !nchunks) return TJ_EINVAL;
+    const int R = sweep_R(tt_only ? M_TT : (M_TT | M_TE | M_EE | M_EB), false, 1, lmax, false, 2);
+    *nchunks = chunk_plan(lmax, R, nparts, h_bounds, h_owner);
+    return TJ_OK;
+}
+
+}  // extern "C"
+
+namespace {
+
+// one device's share of a dense host-buffer call, enqueued but not waited for (tj_coupling_host_part / _multi)
+struct PartCall {
+    double *dw = nullptr, *dout = nullptr;
+    cudaStream_t st = nullptr;
+    int rc = TJ_OK;
+};
+
+// the handle's device must be current
+void part_enqueue(PartCall &pc, const tj_tables *tables, int part, int nparts, int nW, const double *const hw[3],
+                  double *const ho[5], cudaStream_t st)
+{
+    const Tables &T = tables->T;
+    pc.st = st;
+    pc.rc = check_device(tables);
+    if (pc.rc != TJ_OK) return;
+    const size_t N = (size_t)T.lmax + 1, per = N * N;
+    const bool bb_from_ee = (ho[2] && ho[3]);
+    int nout = 0;
+    for (int k = 0; k < 5; ++k) if (ho[k] && !(k == 3 && bb_from_ee)) ++nout;
+    cudaError_t e = cudaMallocAsync((void **)&pc.dw, sizeof(double) * 3 * (size_t)nW, st);
+    if (e == cudaSuccess) e = cudaMallocAsync((void **)&pc.dout, sizeof(double) * per * (size_t)nout, st);
+    const double *dwp[3] = {nullptr, nullptr, nullptr};
+    for (int k = 0; k < 3 && e == cudaSuccess; ++k) {
+        if (!hw[k]) continue;
+        dwp[k] = pc.dw + (size_t)k * nW;
+        e = cudaMemcpyAsync((void *)dwp[k], hw[k], sizeof(double) * (size_t)nW, cudaMemcpyHostToDevice, st);
+    }
+    if (e != cudaSuccess) { pc.rc = cuda_fail(e, "tj_coupling_host_part/set-up"); return; }
+    double *dop[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+    int j = 0;
+    for (int k = 0; k < 5; ++k)
+        if (ho[k] && !(k == 3 && bb_from_ee)) dop[k] = pc.dout + per * (size_t)(j++);
+    pc.rc = run_coupling_rows_to_host(tables, dwp[0], dwp[1], dwp[2], nW, dop, ho, st, part, nparts);
+}
+
+// frees the part's device memory (stream-ordered) and waits for its stream; the handle's device must be current
+void part_finish(PartCall &pc)
+{
+    if (pc.dout) cudaFreeAsync(pc.dout, pc.st);
+    if (pc.dw) cudaFreeAsync(pc.dw, pc.st);
+    pc.dout = pc.dw = nullptr;
+    cudaError_t es = cudaStreamSynchronize(pc.st);
+    if (pc.rc == TJ_OK && es != cudaSuccess) pc.rc = cuda_fail(es, "tj_coupling_host_part/sync");
+}
+
+int part_args_ok(const tj_tables *tables, int nW, double *const ho[5])
+{
+    if (!tables || nW != tables->T.l3max + 1) return 0;
+    if (!ho[0] && !ho[1] && !ho[2] && !ho[3] && !ho[4]) return 0;
+    return 1;
+}
+
+}  // namespace
+
+extern "C" {
+
+int tj_coupling_host_part(const tj_tables *tables, int part, int nparts, int nW, const double *h_Wtt, const double *h_Wtp,
+                          const double *h_Wpp, double *h_TT, double *h_TE, double *h_EE, double *h_BB, double *h_EB,
+                          void *cuda_stream)
+{
+    const double *hw[3] = {h_Wtt, h_Wtp, h_Wpp};
+    double *ho[5] = {h_TT, h_TE, h_EE, h_BB, h_EB};
+    if (nparts < 1 || nparts > PLAN_MAX_PARTS || part < 0 || part >= nparts || !part_args_ok(tables, nW, ho)) return TJ_EINVAL;
+    PartCall pc;
+    part_enqueue(pc, tables, part, nparts, nW, hw, ho, (cudaStream_t)cuda_stream);
+    part_finish(pc);
+    return pc.rc;
+}
+
+int tj_coupling_host_multi(tj_tables *const *tables, int ndev, int nW, const double *h_Wtt, const double *h_Wtp,
+                           const double *h_Wpp, double *h_TT, double *h_TE, double *h_EE, double *h_BB, double *h_EB,
+                           void *const *cuda_streams)
+{
+    const double *hw[3] = {h_Wtt, h_Wtp, h_Wpp};
+    double *ho[5] = {h_TT, h_TE, h_EE, h_BB, h_EB};
+    if (!tables || ndev < 1 || ndev > PLAN_MAX_PARTS) return TJ_EINVAL;
+    for (int g = 0; g < ndev; ++g) {
+        if (!part_args_ok(tables[g], nW, ho) || tables[g]->T.lmax != tables[0]->T.lmax) return TJ_EINVAL;
+        for (int q = 0; q < g; ++q)
+            if (tables[q] == tables[g]) return TJ_EINVAL;   // one handle per part: each owns the side streams of its share
+    }
+    int dev0 = -1;
+    TJ_CUDA(cudaGetDevice(&dev0), "tj_coupling_host_multi/cudaGetDevice");
+    PartCall pc[PLAN_MAX_PARTS];
+    int rc = TJ_OK;
+    // enqueue every device's share (nothing here waits for a GPU), then wait for them one by one
+    for (int g = 0; g < ndev; ++g) {
+        cudaError_t e = cudaSetDevice(tables[g]->device);
+        if (e != cudaSuccess) { pc[g].rc = cuda_fail(e, "tj_coupling_host_multi/cudaSetDevice"); continue; }
+        part_enqueue(pc[g], tables[g], g, ndev, nW, hw, ho, cuda_streams ? (cudaStream_t)cuda_streams[g] : nullptr);
+    }
+    for (int g = 0; g < ndev; ++g) {
+        if (cudaSetDevice(tables[g]->device) == cudaSuccess) part_finish(pc[g]);
+        if (rc == TJ_OK) rc = pc[g].rc;
+    }
+    cudaSetDevice(dev0);
+    return rc;
 }
 
 int tj_set_host_pipeline(tj_tables *tables, double d2h_bytes_per_s, double fp64_instr_per_s)
@@ -981,8 +1095,46 @@ int run_literal(const tj_tables *tables, const double *d_Wtt, const double *d_Wp
 // copy loop) is copied to the host while chunk k+1 is computed.  Successive chunks alternate between two compute
 // streams so that one chunk's last CTAs overlap the next chunk's first ones; within a chunk the tiles keep the
 // descending (largest-first) order.
+// Row chunks of a matrix shared by nparts devices (tj_chunk_plan): chunks of `rows` = a multiple of lcm(R, 32) rows, few
+// enough that no device gets more than PIPE_MAX_CHUNKS of them, dealt to the devices by work -- the chunk with the most
+// sweep steps (sum over its rows l1 of (l1+1)(N-l1)) first, each to the device with the least work so far, ties to the
+// lower index.  bounds[0..n], owner[0..n-1]; returns n (<= PIPE_MAX_CHUNKS / 2 * nparts).
+int chunk_plan(int lmax, int R, int nparts, int *bounds, int *owner)
+{
+    const long long N = (long long)lmax + 1;
+    int L = R;
+    while (L % 32) L += R;
+    const long long units = (N + L - 1) / L;
+    const long long cap = (long long)(PIPE_MAX_CHUNKS / 2) * nparts;   // 12 per device on average, never more than 24
+    const long long rows = L * ((units + cap - 1) / cap);
+    const int n = (int)((N + rows - 1) / rows);
+    double work[PIPE_MAX_CHUNKS / 2 * PLAN_MAX_PARTS];
+    for (int k = 0; k <= n; ++k) bounds[k] = (int)(k * rows < N ? k * rows : N);
+    for (int k = 0; k < n; ++k) {
+        double w = 0.0;
+        for (long long l = bounds[k]; l < bounds[k + 1]; ++l) w += (double)(l + 1) * (double)(N - l);
+        work[k] = w;
+        owner[k] = -1;
+    }
+    double load[PLAN_MAX_PARTS] = {0.0};
+    int count[PLAN_MAX_PARTS] = {0};
+    for (int it = 0; it < n; ++it) {
+        int best = -1;
+        for (int k = 0; k < n; ++k)
+            if (owner[k] < 0 && (best < 0 || work[k] > work[best])) best = k;
+        int g = -1;
+        for (int q = 0; q < nparts; ++q)
+            if (count[q] < PIPE_MAX_CHUNKS && (g < 0 || load[q] < load[g])) g = q;
+        owner[best] = g;
+        load[g] += work[best];
+        ++count[g];
+    }
+    return n;
+}
+
 int run_coupling_rows_to_host(const tj_tables *tables, const double *d_Wtt, const double *d_Wtp, const double *d_Wpp,
-                              int nW, double *const d_out[5], double *const h_out[5], cudaStream_t st)
+                              int nW, double *const d_out[5], double *const h_out[5], cudaStream_t st, int part,
+                              int nparts)
 {
     HostPipe &pipe = const_cast<tj_tables *>(tables)->pipe;
     std::lock_guard<std::mutex> lock(pipe.mu);
@@ -1004,7 +1156,8 @@ int run_coupling_rows_to_host(const tj_tables *tables, const double *d_Wtt, cons
     const double copy_s = (double)nmat_host * (double)C.N * (double)C.N * 8.0 / pipe.copy_rate;
     const double n3 = (double)C.N * (double)C.N * (double)C.N / 6.0;   // even (and odd) steps of the upper triangle
     const double comp_s = (C.mask == M_TT ? 2.0 : 13.0) * n3 / pipe.instr_rate;
-    const bool rows_mode = copy_s > comp_s;
+    // one part of several (tj_coupling_host_part / _multi): only the L-shaped regions are self-contained per chunk
+    const bool rows_mode = nparts == 1 && copy_s > comp_s;
     // chunk ends as fractions of the rows.  Compute-bound: a first chunk of 20 % of the rows is 10 % of the work and
     // releases 36 % of the bytes (measured at config 3: 4 chunks 163 ms, 6 chunks 145 ms, these 10 chunks 135.4 ms;
     // device-buffer call 134.4 ms).  Copy-bound: 1 % first (the copy engine starts at once), then even steps; measured
@@ -1030,7 +1183,18 @@ int run_coupling_rows_to_host(const tj_tables *tables, const double *d_Wtt, cons
         long long r = (k == nfrac - 1) ? C.N : (long long)(frac[k] * (double)C.N) / L * L;
         if (r > bound[nchunk]) bound[++nchunk] = (int)r;
     }
-    pipe.last_regime = rows_mode ? 1 : 2;
+    // several parts: this part's chunks of the shared plan, in ascending row order (each with its own two bounds)
+    int own_lo[PIPE_MAX_CHUNKS], own_hi[PIPE_MAX_CHUNKS];
+    if (nparts > 1) {
+        int pb[PIPE_MAX_CHUNKS / 2 * PLAN_MAX_PARTS + 1], po[PIPE_MAX_CHUNKS / 2 * PLAN_MAX_PARTS];
+        const int n = chunk_plan(C.T->lmax, C.R, nparts, pb, po);
+        nchunk = 0;
+        for (int k = 0; k < n; ++k)
+            if (po[k] == part) { own_lo[nchunk] = pb[k]; own_hi[nchunk] = pb[k + 1]; ++nchunk; }
+    } else {
+        for (int k = 0; k < nchunk; ++k) { own_lo[k] = bound[k]; own_hi[k] = bound[k + 1]; }
+    }
+    pipe.last_regime = nparts > 1 ? 4 : rows_mode ? 1 : 2;
     pipe.last_chunks = nchunk;
     cudaEvent_t *ev = pipe.ev;
     cudaEvent_t fork = ev[PIPE_MAX_CHUNKS], join = ev[PIPE_MAX_CHUNKS + 1];
@@ -1038,7 +1202,7 @@ int run_coupling_rows_to_host(const tj_tables *tables, const double *d_Wtt, cons
     for (int k = 0; k < 2 && e == cudaSuccess; ++k) e = cudaStreamWaitEvent(pipe.comp[k], fork, 0);
     if (e == cudaSuccess) e = cudaStreamWaitEvent(pipe.copy, fork, 0);
     for (int k = 0; k < nchunk && e == cudaSuccess; ++k) {
-        const int r0 = bound[k], r1 = bound[k + 1];
+        const int r0 = own_lo[k], r1 = own_hi[k];
         // successive chunks alternate between two compute streams: one chunk's last CTAs overlap the next one's first
         cudaStream_t cs = pipe.comp[k & 1];
         const int b1 = (r1 == C.N) ? C.nb : r1 / C.R;

@@ -150,6 +150,80 @@ def test_one_handle_from_two_threads_host_and_device_calls():
     T.close()
 
 
+# ---------------------------------------------------------------- one matrix on several devices, every pair swept once
+def _plan_mask(lmax, nparts, part, tt_only=False):
+    import torch
+    bounds, owner = binding.chunk_plan(lmax, nparts, tt_only=tt_only)
+    N = lmax + 1
+    m = torch.zeros((N, N), dtype=torch.bool)
+    for k, g in enumerate(owner):
+        if g == part:
+            r0, r1 = bounds[k], bounds[k + 1]
+            m[r0:r1, r0:] = True
+            m[r1:, r0:r1] = True
+    return m
+
+
+@pytest.mark.parametrize("lmax,nparts,keys", [(1000, 2, BLOCKS), (2700, 4, BLOCKS), (1500, 3, ("TT",)), (300, 2, ("EE", "EB"))])
+def test_host_parts_one_after_the_other_complete_the_matrix_bitwise(lmax, nparts, keys):
+    """tj_coupling_host_part for part = 0..nparts-1 into ONE set of host matrices (here one after the other on one GPU;
+    on nparts GPUs the same calls run side by side): each call writes exactly the regions of its own chunks and nothing
+    else, and together they give the bits of the whole-matrix call."""
+    import torch
+    wl, hw = _problem(lmax)
+    N = lmax + 1
+    T = binding.build_tables(lmax)
+    dev = [w.cuda() for w in hw]
+    tt_only = keys == ("TT",)
+    pol = not tt_only
+    ref = binding.coupling_pol(T, dev[0] if "TT" in keys else None, dev[1] if "TE" in keys else None,
+                               dev[2] if pol else None, want=keys)
+    torch.cuda.synchronize()
+    ref = {k: v.cpu() for k, v in ref.items()}
+    pw = [w.pin_memory() for w in hw]
+    args = (pw[0] if "TT" in keys else None, pw[1] if "TE" in keys else None, pw[2] if pol else None)
+    out = _nan_out(N, keys)
+    done = torch.zeros((N, N), dtype=torch.bool)
+    for part in range(nparts):
+        binding.coupling_host_part(T, part, nparts, *args, out)
+        assert binding.host_pipeline_info(T)[0] == 4
+        mine = _plan_mask(lmax, nparts, part, tt_only=tt_only)
+        assert not bool((done & mine).any())
+        done |= mine
+        for k in keys:
+            assert bool(torch.isnan(out[k][~done]).all()), (part, k)          # nothing outside the parts run so far
+            assert torch.equal(out[k][mine], ref[k][mine]), (part, k)
+    assert bool(done.all())
+    for k in keys:
+        assert torch.equal(out[k], ref[k]), k
+    with pytest.raises(binding.TJError):
+        binding.coupling_host_part(T, nparts, nparts, *args, out)
+    T.close()
+
+
+def test_host_multi_with_three_handles_on_one_gpu_bitwise():
+    """tj_coupling_host_multi with three handles ("virtual ranks": all on this one GPU, each with its own stream and side
+    streams), running side by side: the one set of host matrices is complete and carries the bits of the single call."""
+    import torch
+    lmax = 2700
+    wl, hw = _problem(lmax, cfg=3)
+    N = lmax + 1
+    Ts = [binding.build_tables(lmax) for _ in range(3)]
+    ref = binding.coupling_pol(Ts[0], *[w.cuda() for w in hw])
+    torch.cuda.synchronize()
+    pw = [w.pin_memory() for w in hw]
+    for streams in (None, [torch.cuda.Stream() for _ in range(3)]):
+        out = _nan_out(N, BLOCKS)
+        binding.coupling_host_multi(Ts, *pw, out, streams=streams)
+        for k in BLOCKS:
+            assert torch.equal(out[k].cuda(), ref[k]), k
+        assert [binding.host_pipeline_info(t)[0] for t in Ts] == [4, 4, 4]
+    with pytest.raises(binding.TJError):      # the same handle twice
+        binding.coupling_host_multi([Ts[0], Ts[0]], *pw, _nan_out(N, BLOCKS))
+    for t in Ts:
+        t.close()
+
+
 def test_profiled_calls_keep_their_status_and_times_per_thread():
     """Per-kernel profiling is per thread: a thread that has made no profiled call gets TJ_EINVAL from tj_profile_get,
     and profiling never changes a call's result."""
@@ -258,3 +332,27 @@ def test_two_devices_from_two_threads():
     for t in th:
         t.join()
     assert not errors, errors
+
+
+def test_host_multi_on_two_devices():
+    """tj_coupling_host_multi with one handle per GPU: the one set of host matrices carries the bits of the single call."""
+    import torch
+    if not _two_gpus():
+        pytest.skip("needs two GPUs")
+    lmax = 2700
+    N = lmax + 1
+    wl, hw = _problem(lmax, cfg=3)
+    Ts = []
+    for d in (0, 1):
+        with torch.cuda.device(d):
+            Ts.append(binding.build_tables(lmax))
+    with torch.cuda.device(0):
+        ref = {k: v.cpu() for k, v in binding.coupling_pol(Ts[0], *[w.cuda() for w in hw]).items()}
+        out = _nan_out(N, BLOCKS)
+        binding.coupling_host_multi(Ts, *[w.pin_memory() for w in hw], out)
+        assert torch.cuda.current_device() == 0
+    for k in BLOCKS:
+        assert torch.equal(out[k], ref[k]), k
+    for d in (0, 1):
+        with torch.cuda.device(d):
+            Ts[d].close()

@@ -142,3 +142,90 @@ def test_row_blocks_partition_is_a_balanced_cover():
             assert max(loads) <= 1.02 * sum(cost) / world + max(cost)
     with pytest.raises(ValueError):
         shard.row_blocks(10, 0)
+
+
+# ---------------------------------------------------------------- one matrix on several GPUs, every pair swept once (tj_chunk_plan)
+def _region_mask(N, r0, r1):
+    """The L-shaped region chunk [r0, r1) makes final (include/tj.h): its rows from column r0 on, and columns [r0, r1)
+    of all rows below."""
+    m = torch.zeros((N, N), dtype=torch.int32)
+    m[r0:r1, r0:] = 1
+    m[r1:, r0:r1] = 1
+    return m
+
+
+def _chunks_worker(rank, world, port, lmax, q):
+    sys.path.insert(0, ROOT)
+    from paper_2602_15605_b200 import binding, build
+    build.build()
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    bounds, owner = binding.chunk_plan(lmax, world)          # host-side entry point of libtj: no GPU involved
+    N = lmax + 1
+    stored = torch.zeros((N, N), dtype=torch.int32)
+    swept = torch.zeros((N, N), dtype=torch.int32)
+    l1 = torch.arange(N)[:, None]
+    l2 = torch.arange(N)[None, :]
+    work = 0
+    for k, g in enumerate(owner):
+        if g != rank:
+            continue
+        r0, r1 = bounds[k], bounds[k + 1]
+        stored += _region_mask(N, r0, r1)
+        swept += ((l1 >= r0) & (l1 < r1) & (l2 >= l1)).to(torch.int32)   # the chunk's sweep: its rows of the upper triangle
+        work += sum((a + 1) * (N - a) for a in range(r0, r1))
+    tot_stored, tot_swept = stored.clone(), swept.clone()
+    dist.all_reduce(tot_stored)
+    dist.all_reduce(tot_swept)
+    works = [None] * world
+    dist.all_gather_object(works, work)
+    q.put((rank, tot_stored, tot_swept, works, (bounds, owner)))
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("lmax", [700, 2700])
+def test_chunk_ownership_stores_every_entry_once_and_sweeps_every_pair_once_world2(lmax):
+    world = 2
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_chunks_worker, args=(r, world, port, lmax, q)) for r in range(world)]
+    for p in procs:
+        p.start()
+    res = [q.get(timeout=180) for _ in range(world)]
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    N = lmax + 1
+    assert res[0][4] == res[1][4]                                              # both ranks derive the same plan
+    for rank, tot_stored, tot_swept, works, _ in res:
+        assert bool((tot_stored == 1).all())                                   # every (l1,l2) delivered by exactly one rank
+        upper = torch.arange(N)[None, :] >= torch.arange(N)[:, None]
+        assert bool((tot_swept[upper] == 1).all()) and bool((tot_swept[~upper] == 0).all())   # no pair swept twice
+        assert max(works) <= 1.05 * min(works)
+
+
+def test_chunk_plan_is_a_balanced_cover_for_any_device_count():
+    from paper_2602_15605_b200 import binding, build
+    build.build()
+    for lmax, tt in [(0, False), (31, False), (800, False), (2599, False), (2600, False), (5000, True), (10000, False)]:
+        N = lmax + 1
+        unit = 96 if (lmax >= 2600 and not tt) else 32
+        for G in (1, 2, 3, 4, 8, 64):
+            bounds, owner = binding.chunk_plan(lmax, G, tt_only=tt)
+            assert bounds[0] == 0 and bounds[-1] == N and all(a < b for a, b in zip(bounds, bounds[1:]))
+            assert all(b % unit == 0 for b in bounds[:-1])                   # whole row bands and whole writer tile rows
+            assert len(owner) == len(bounds) - 1 <= 12 * G and all(0 <= g < G for g in owner)
+            per = [sum(1 for g in owner if g == d) for d in range(G)]
+            assert max(per) <= 24
+            load = [0] * G
+            for k, g in enumerate(owner):
+                load[g] += sum((a + 1) * (N - a) for a in range(bounds[k], bounds[k + 1]))
+            if lmax == 10000 and G <= 8:
+                assert max(load) <= 1.01 * sum(load) / G                     # config 3: within 1 % on 8 GPUs
+    with pytest.raises(binding.TJError):
+        binding.chunk_plan(100, 0)
+    with pytest.raises(binding.TJError):
+        binding.chunk_plan(100, 65)
